@@ -1,0 +1,288 @@
+"""CPU ORACLE — test infrastructure, NOT a product path.
+
+Plain float64 / int64 NumPy restatement of the sparse-CSR preprocessing chain
+of arxiv/paper_2603_02402 (rapids-singlecell): per-cell / per-gene QC,
+normalize_total, log1p, per-gene moments and Seurat-flavour highly-variable-gene
+selection.  Every function is the plain definition of what the step computes,
+one pass per quantity, no blocking / fusion / reordering, so that it can be
+checked against the paper by eye.  It shares no code with the CUDA path
+(`paper_2603_02402_b200/csrc`) and imports nothing from the package.
+
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s `cpu_baseline` /
+`--impl reference` legs may import this module.
+
+Citations are `PAPER.md:L<line>` (the only reference file) plus the section.
+Where the paper is silent the reading of DESIGN.md §3 (R1..R15) is followed
+and named.
+
+Pins (tests/test_oracle_*.py, `-m "not gpu"`):
+  qc_metrics       dense brute force, scipy.sparse reductions, sum invariants
+  normalize_total  row sums == target_sum, dense brute force, s == T identity
+  log1p            numpy.log1p on the dense matrix, expm1 round trip, pattern kept
+  gene_moments     np.mean / np.var(ddof) on the dense matrix, closed forms
+  hvg_select       H3/H4 against pandas.cut; per-bin z mean 0 / sd 1; single-gene
+                   bin => z == 1; brute-force loops on tiny inputs; hand-worked
+                   fixture tests/golden/hvg_tiny.txt.
+  The CONSTANTS of H1/H5 (1e-12 floor, 0.1 % edge extension, ddof = 1 inside
+  bins, z = 1 rule) are not in PAPER.md ("follows scanpy", L87) and scanpy is
+  not installed: those constants are **parity unpinned** against the paper.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+F32 = np.float32
+F64 = np.float64
+I64 = np.int64
+I32 = np.int32
+
+
+def _row_ids(indptr: np.ndarray) -> np.ndarray:
+    """i(p): the row of every stored entry."""
+    indptr = np.asarray(indptr, dtype=I64)
+    n = indptr.shape[0] - 1
+    return np.repeat(np.arange(n, dtype=I64), np.diff(indptr))
+
+
+def _int_sum(groups: np.ndarray, values_i64: np.ndarray, size: int) -> np.ndarray:
+    """Exact int64 group sums (float64 bincount is exact below 2**53)."""
+    w = values_i64.astype(F64)
+    out = np.bincount(groups, weights=w, minlength=size)
+    assert np.all(np.abs(out) < 2.0 ** 53), "integer sum not exactly representable"
+    return out.astype(I64)
+
+
+# --------------------------------------------------------------------------
+# Q1..Q4  QC metrics  ("QC metrics" cell-wise on CSR; L17/L21
+# "filtering"; the list of metrics is reading R1)
+# --------------------------------------------------------------------------
+def qc_metrics(indptr, indices, data, n_genes: int, gene_flags=None) -> dict:
+    """Per-cell and per-gene QC reductions.
+
+    Q1  T_i  = sum_{p in row i} (int64) x_p                 total_counts
+    Q2  N_i  = #{p in row i : x_p != 0}                      n_genes_by_counts
+    Q3  M_i  = sum_{p in row i, flag[j(p)] != 0} (int64) x_p ; pct_i = 100 M_i / T_i
+    Q4  C_j  = #{p : j(p) = j, x_p != 0} ;  T_j = sum_{p: j(p)=j} (int64) x_p
+    "detected" means value != 0, not "stored" (R2).  T_i == 0 -> pct NaN (R3).
+    Totals are int64 sums of the truncated values (R4).
+    """
+    indptr = np.asarray(indptr, dtype=I64)
+    indices = np.asarray(indices, dtype=I64)
+    data = np.asarray(data, dtype=F32)
+    n = indptr.shape[0] - 1
+    rows = _row_ids(indptr)
+    xi = data.astype(F64).astype(I64)            # (int64) x_p, truncation
+    nzmask = data != 0
+
+    cell_total = _int_sum(rows, xi, n)
+    cell_n_genes = np.bincount(rows[nzmask], minlength=n).astype(I32)
+    if gene_flags is None:
+        cell_flag_total = np.zeros(n, dtype=I64)
+    else:
+        fl = np.asarray(gene_flags) != 0
+        sel = fl[indices]
+        cell_flag_total = _int_sum(rows[sel], xi[sel], n)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        pct = (100.0 * cell_flag_total.astype(F64) / cell_total.astype(F64)).astype(F32)
+
+    gene_n_cells = np.bincount(indices[nzmask], minlength=n_genes).astype(I32)
+    gene_total = _int_sum(indices, xi, n_genes)
+    return dict(
+        cell_total_i64=cell_total,
+        cell_total_f32=cell_total.astype(F32),
+        cell_n_genes=cell_n_genes,
+        cell_flag_total_i64=cell_flag_total,
+        cell_flag_pct=pct,
+        gene_n_cells=gene_n_cells,
+        gene_total_i64=gene_total,
+    )
+
+
+# --------------------------------------------------------------------------
+# N1  normalize_total   PAPER.md:L91  x'_ij = (x_ij / sum_j x_ij) * s
+# --------------------------------------------------------------------------
+def normalize_total(indptr, data, target_sum: float, cell_total_i64=None):
+    """Returns (x' as float32, scale float64[n]).
+
+    scale_i = s / T_i in float64; x'_p = (float32)((double)x_p * scale_i): one
+    rounding (R5).  A cell with T_i == 0 is left untouched, scale 1 (R3).
+    When totals are not supplied they are the float64 row sums of the data.
+    """
+    indptr = np.asarray(indptr, dtype=I64)
+    data = np.asarray(data, dtype=F32)
+    n = indptr.shape[0] - 1
+    rows = _row_ids(indptr)
+    if cell_total_i64 is None:
+        tot = np.bincount(rows, weights=data.astype(F64), minlength=n)
+    else:
+        tot = np.asarray(cell_total_i64).astype(F64)
+    scale = np.ones(n, dtype=F64)
+    ok = tot != 0
+    scale[ok] = F64(target_sum) / tot[ok]
+    out = (data.astype(F64) * scale[rows]).astype(F32)
+    return out, scale
+
+
+# --------------------------------------------------------------------------
+# L1  log1p   PAPER.md:L91  x''_ij = log(1 + x'_ij), natural log (R7)
+# --------------------------------------------------------------------------
+def log1p(data):
+    return np.log1p(np.asarray(data, dtype=F32).astype(F64)).astype(F32)
+
+
+# --------------------------------------------------------------------------
+# M1  per-gene moments   PAPER.md:L91 "per-gene mean and variance ... custom GPU
+# reduction kernel that operates directly on sparse matrices"; L137.
+# --------------------------------------------------------------------------
+def gene_moments(indptr, indices, data, n_genes: int, transform: int = 0, ddof: int = 1):
+    """mean_j, var_j over ALL n cells (zeros included), float64.
+
+    v_p = x_p (transform 0) or expm1(x_p) (transform 1, reading R8).
+    mean_j = (1/n) sum_p v_p ;
+    var_j  = ( sum_{stored} (v_p - mean_j)^2 + (n - nnz_j) mean_j^2 ) / (n - ddof)
+    i.e. the textbook two-pass variance of the dense column; ddof = 1 is the
+    (n-1) convention the paper uses for its covariance (L95, reading R11).
+    Returns (mean, var, S1, S2) with S1 = sum v, S2 = sum v^2.
+    """
+    indptr = np.asarray(indptr, dtype=I64)
+    indices = np.asarray(indices, dtype=I64)
+    n = indptr.shape[0] - 1
+    v = np.asarray(data, dtype=F32).astype(F64)
+    if transform == 1:
+        v = np.expm1(v)
+    elif transform != 0:
+        raise ValueError("transform must be 0 or 1")
+    s1 = np.bincount(indices, weights=v, minlength=n_genes)
+    s2 = np.bincount(indices, weights=v * v, minlength=n_genes)
+    stored = np.bincount(indices, minlength=n_genes).astype(F64)
+    mean = s1 / F64(n) if n > 0 else np.zeros(n_genes)
+    dev = v - mean[indices]
+    ss = np.bincount(indices, weights=dev * dev, minlength=n_genes)
+    ss = ss + (F64(n) - stored) * mean * mean
+    with np.errstate(divide="ignore", invalid="ignore"):
+        var = ss / F64(n - ddof)
+    return mean, var, s1, s2
+
+
+# --------------------------------------------------------------------------
+# H1..H7  Seurat-flavour HVG selection.  PAPER.md:L91 "Highly variable gene
+# selection is based on per-gene mean and variance"; L39 "gene selection"
+# kernel; L87 "follow the algorithmic implementations of scanpy".  The steps
+# are reading R8/R9/R10/R12; their constants are parity
+# unpinned against PAPER.md (see module header).
+# --------------------------------------------------------------------------
+def bin_edges(m: np.ndarray, n_bins: int) -> np.ndarray:
+    """H3: n_bins equal-width, right-closed bins over [min m, max m].
+
+    step = (hi - lo)/n_bins ; edge_k = fl(fl(k*step) + lo) for k < n_bins ;
+    edge_{n_bins} = hi ; then edge_0 -= 0.001*(hi - lo).
+    Degenerate hi == lo (R10): lo -= 0.001*|lo| (or 0.001 when lo == 0),
+    hi += 0.001*|hi| (or 0.001), no further extension.
+    """
+    m = np.asarray(m, dtype=F64)
+    lo = F64(np.min(m))
+    hi = F64(np.max(m))
+    degenerate = lo == hi
+    if degenerate:
+        lo = lo - (F64(0.001) * abs(lo) if lo != 0 else F64(0.001))
+        hi = hi + (F64(0.001) * abs(hi) if hi != 0 else F64(0.001))
+    step = (hi - lo) / F64(n_bins)
+    edges = np.empty(n_bins + 1, dtype=F64)
+    for k in range(n_bins):
+        edges[k] = F64(k) * step + lo       # two roundings, no fused multiply-add
+    edges[n_bins] = hi
+    if not degenerate:
+        edges[0] = edges[0] - (hi - lo) * F64(0.001)
+    return edges
+
+
+def assign_bins(m: np.ndarray, edges: np.ndarray) -> np.ndarray:
+    """H4: bin(m) = smallest k with m <= edge_{k+1}  (intervals (edge_k, edge_{k+1}])."""
+    m = np.asarray(m, dtype=F64)
+    nb = edges.shape[0] - 1
+    out = np.empty(m.shape[0], dtype=I32)
+    for g in range(m.shape[0]):
+        k = 0
+        while k < nb - 1 and not (m[g] <= edges[k + 1]):
+            k += 1
+        out[g] = k
+    return out
+
+
+def hvg_select(gene_mean, gene_var, n_top: int, n_bins: int = 20, seurat_log: bool = True) -> dict:
+    """H1..H7.  Inputs: per-gene mean and variance (float64).
+
+    H1  mean == 0 -> 1e-12 ;  d = var / mean
+    H2  (seurat_log) d == 0 -> NaN ; d = ln d ; m = log1p(mean)
+    H3/H4  20 equal-width bins over m, right-closed
+    H5  per bin: mu_b = mean of the non-NaN d, sigma_b = their sample sd (ddof 1);
+        exactly one non-NaN gene in the bin -> sigma_b = mu_b, mu_b = 0 (z = 1)
+    H6  z = (d - mu_b) / sigma_b
+    H7  cutoff = n_top-th largest non-NaN z (all of them if fewer, R12);
+        mask = z >= cutoff (ties at the cutoff are all selected)
+    """
+    mean = np.array(gene_mean, dtype=F64, copy=True)
+    var = np.asarray(gene_var, dtype=F64)
+    G = mean.shape[0]
+    mean[mean == 0] = F64(1e-12)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        d = var / mean
+        if seurat_log:
+            d = np.where(d == 0, np.nan, d)
+            d = np.log(d)
+            m = np.log1p(mean)
+        else:
+            m = mean.copy()
+    edges = bin_edges(m, n_bins)
+    b = assign_bins(m, edges)
+
+    mu_b = np.full(n_bins, np.nan)
+    sd_b = np.full(n_bins, np.nan)
+    for k in range(n_bins):
+        dk = d[b == k]
+        dk = dk[~np.isnan(dk)]
+        if dk.shape[0] == 0:
+            continue
+        mk = np.sum(dk) / F64(dk.shape[0])
+        if dk.shape[0] == 1:
+            mu_b[k] = 0.0
+            sd_b[k] = mk
+        else:
+            mu_b[k] = mk
+            sd_b[k] = np.sqrt(np.sum((dk - mk) ** 2) / F64(dk.shape[0] - 1))
+    with np.errstate(divide="ignore", invalid="ignore"):
+        z = (d - mu_b[b]) / sd_b[b]
+
+    valid = ~np.isnan(z)
+    n_valid = int(valid.sum())
+    k = min(int(n_top), n_valid)
+    if k > 0:
+        zs = np.sort(z[valid])[::-1]
+        cutoff = zs[k - 1]
+        mask = valid & (z >= cutoff)
+    else:
+        cutoff = np.nan
+        mask = np.zeros(G, dtype=bool)
+    idx = np.nonzero(mask)[0].astype(I32)
+    return dict(mean_t=m, disp=d, disp_norm=z, bin=b, edges=edges,
+                mask=mask.astype(np.uint8), indices=idx, count=int(idx.shape[0]),
+                cutoff=cutoff)
+
+
+# --------------------------------------------------------------------------
+# The chain as the paper orders it (QC -> normalize ->
+# log1p -> HVG).  Composition only; no arithmetic of its own.
+# --------------------------------------------------------------------------
+def preprocess_chain(indptr, indices, data, n_genes, gene_flags, target_sum, n_top,
+                     n_bins=20, ddof=1, hvg_on="linear") -> dict:
+    qc = qc_metrics(indptr, indices, data, n_genes, gene_flags)
+    xn, scale = normalize_total(indptr, data, target_sum, qc["cell_total_i64"])
+    xl = log1p(xn)
+    mean_log, var_log, _, _ = gene_moments(indptr, indices, xl, n_genes, 0, ddof)
+    mean_lin, var_lin, _, _ = gene_moments(indptr, indices, xn, n_genes, 0, ddof)
+    if hvg_on == "linear":
+        hv = hvg_select(mean_lin, var_lin, n_top, n_bins)
+    else:
+        hv = hvg_select(mean_log, var_log, n_top, n_bins)
+    return dict(qc=qc, x_norm=xn, x_log=xl, mean_log=mean_log, var_log=var_log,
+                mean_lin=mean_lin, var_lin=var_lin, hvg=hv)
