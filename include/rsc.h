@@ -1,0 +1,232 @@
+/*
+ * rsc.h — C ABI of librsc_b200: the sparse-CSR single-cell preprocessing chain of
+ * arxiv/paper_2603_02402 (rapids-singlecell) as hand-written sm_100a CUDA kernels.
+ *
+ * The chain (PAPER.md:L47, L145 workflow order; L85 "CSR format is used for
+ * cell-wise operations (e.g., normalization, QC metrics)"; L91 "Preprocessing and
+ * normalization"):
+ *     QC reductions -> normalize_total -> log1p -> per-gene moments -> HVG selection
+ *
+ * Conventions (all entry points)
+ *   - Pointers are DEVICE pointers owned by the caller unless the name says `host`.
+ *     The library never allocates or frees device memory and never synchronises
+ *     the stream: every call only enqueues work on `stream` (a cudaStream_t passed
+ *     as void*; NULL = the legacy default stream) and returns.
+ *   - Scratch memory comes from the caller: `ws` must hold at least the number of
+ *     bytes the matching `*_workspace_bytes` query returns and be 256-byte aligned.
+ *     Its contents are undefined on entry and on exit.
+ *   - Return value: RSC_OK or a negative rsc_status.  After a failure
+ *     rsc_last_error() returns a thread-local, human-readable description.
+ *     Arguments are validated on the host; the matrix CONTENT is not validated
+ *     (canonical CSR is a precondition: indptr non-decreasing with indptr[0]=0 and
+ *     indptr[n_rows]=nnz, 0 <= indices < n_cols, no duplicate column inside a row).
+ *   - Optional outputs may be NULL and are then skipped.
+ *   - Matrix layout: float32 `data`, int32 `indices`, int64 `indptr`
+ *     (BASELINE.json north_star; int64 lifts the ~2^31 nnz ceiling of PAPER.md:L43,
+ *     L141).
+ */
+#ifndef RSC_H_
+#define RSC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  RSC_OK = 0,
+  RSC_ERR_INVALID_ARG = -1, /* NULL required pointer, negative size, bad parameter   */
+  RSC_ERR_WORKSPACE = -2,   /* workspace too small or misaligned                     */
+  RSC_ERR_CUDA = -3,        /* CUDA runtime / launch error (text in rsc_last_error)  */
+  RSC_ERR_UNSUPPORTED = -4  /* current device is not compute capability 10.x         */
+} rsc_status;
+
+/* rsc_csr.flags */
+#define RSC_CSR_SORTED 1 /* column indices strictly ascending inside every row.  Enables the
+                            conflict-free shared-memory accumulation path; without it the
+                            kernels fall back to L2 atomics (same results, slower).          */
+
+typedef struct {
+  int64_t n_rows;        /* cells n                                                   */
+  int32_t n_cols;        /* genes G                                                   */
+  int32_t flags;         /* RSC_CSR_* bits                                            */
+  int64_t nnz;           /* == indptr[n_rows]; passed by the caller to avoid a sync   */
+  const int64_t* indptr; /* [n_rows + 1]                                              */
+  const int32_t* indices;/* [nnz]                                                     */
+  float* data;           /* [nnz]; rewritten in place by normalize / log1p / fused    */
+} rsc_csr;
+
+const char* rsc_last_error(void);
+/* Library version, "major.minor.patch". */
+const char* rsc_version(void);
+/* Number of CUDA kernels this library has launched so far in the calling process (host-side
+ * counter; memsets / memcpys are not counted).  Used by bench.py to report gpu_launches. */
+uint64_t rsc_kernel_launch_count(void);
+
+/* ---------------------------------------------------------------------------------
+ * rsc_qc_metrics — per-cell and per-gene QC reductions.
+ * PAPER.md:L85 ("QC metrics", cell-wise on CSR), L17/L21 ("filtering"); the list of
+ * metrics is BASELINE.json north_star's (reading R1).
+ *   cell_total_i64[i]      T_i = sum over row i of (int64) x          (exact integer)
+ *   cell_total_f32[i]      (float) T_i
+ *   cell_n_genes[i]        #{stored entries of row i with x != 0}
+ *   cell_flag_total_i64[i] M_i = sum over row i, gene_flags[col] != 0, of (int64) x
+ *   cell_flag_pct[i]       (float)(100.0 * M_i / T_i) evaluated in double; NaN when T_i = 0
+ *   gene_n_cells[j]        #{stored entries of column j with x != 0}
+ *   gene_total_i64[j]      sum over column j of (int64) x
+ * Values are truncated to integers before summation; counts must be < 2^24.
+ * gene_flags: uint8[n_cols] or NULL (then M_i = 0, pct = 0 or NaN).
+ * Outputs are fully overwritten (no accumulation into previous contents).
+ * ------------------------------------------------------------------------------- */
+size_t rsc_qc_metrics_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
+int rsc_qc_metrics(const rsc_csr* X, const uint8_t* gene_flags,
+                   int64_t* cell_total_i64, float* cell_total_f32, int32_t* cell_n_genes,
+                   int64_t* cell_flag_total_i64, float* cell_flag_pct,
+                   int32_t* gene_n_cells, int64_t* gene_total_i64,
+                   void* ws, size_t ws_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------
+ * rsc_normalize_total — PAPER.md:L91  x'_ij = (x_ij / sum_j x_ij) * s, in place.
+ *   scale_i = target_sum / (float) T_i  (float32 division), data[p] *= scale_i.
+ *   cell_total_i64: T_i from rsc_qc_metrics, or NULL -> the kernel sums each row
+ *   itself (double accumulation of the float values).
+ *   A row with T_i == 0 is left untouched (scale 1).
+ *   cell_scale_out: optional float[n_rows] receiving scale_i.
+ *   target_sum must be finite and > 0.
+ * ------------------------------------------------------------------------------- */
+int rsc_normalize_total(rsc_csr* X, float target_sum, const int64_t* cell_total_i64,
+                        float* cell_scale_out, void* stream);
+
+/* ---------------------------------------------------------------------------------
+ * rsc_log1p — PAPER.md:L91  x''_ij = log(1 + x'_ij) (natural log), in place on
+ * X->data; indptr / indices are not touched, log1p(0) = 0 keeps the pattern.
+ * ------------------------------------------------------------------------------- */
+int rsc_log1p(rsc_csr* X, void* stream);
+
+/* ---------------------------------------------------------------------------------
+ * rsc_gene_moments — PAPER.md:L91 / L137 "per-gene reduction kernels for mean and
+ * variance" operating directly on the sparse matrix (no CSC copy, cf. L85).
+ *   v = data[p] (transform 0) or expm1((double)data[p]) (transform 1)
+ *   S1_j = sum v, S2_j = sum v^2 in double precision over the stored entries,
+ *   mean_j = S1_j / n,  var_j = max(0, (S2_j - n mean_j^2) / (n - ddof)); zeros are
+ *   included through n.  ddof in {0, 1}; n - ddof must be > 0.
+ *   gene_sum / gene_sumsq: optional double[n_cols] receiving S1 / S2.
+ * ------------------------------------------------------------------------------- */
+size_t rsc_gene_moments_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
+int rsc_gene_moments(const rsc_csr* X, int transform, int ddof,
+                     double* gene_mean, double* gene_var,
+                     double* gene_sum, double* gene_sumsq,
+                     void* ws, size_t ws_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------
+ * rsc_normalize_log1p_moments — the fused pass (BASELINE.json north_star; not in the
+ * paper, which runs L91's three steps as separate kernels): every stored entry is
+ * read once, x' = x * scale_i, x'' = log1p(x') is written back, and the per-gene
+ * sums of the ROUNDED float32 x'' (log scale) and/or x' (linear scale) are
+ * accumulated in double precision.
+ *   which_moments: bit0 RSC_MOMENTS_LOG -> mean_log/var_log, bit1 RSC_MOMENTS_LIN ->
+ *   mean_lin/var_lin (the matching pointers are then required).
+ *   cell_total_i64 is required (from rsc_qc_metrics).
+ *   gene_n_cells: optional hint (from rsc_qc_metrics) used to balance the gene
+ *   ranges of the shared-memory accumulators; results do not depend on it.
+ *   gene_sums_out: optional double[4 * n_cols] receiving the raw sums
+ *   S1log | S2log | S1lin | S2lin (n_cols each; only the requested sets are written).
+ *   Row-sharded multi-GPU runs all-reduce these and call rsc_moments_finalize.
+ * ------------------------------------------------------------------------------- */
+#define RSC_MOMENTS_LOG 1
+#define RSC_MOMENTS_LIN 2
+size_t rsc_normalize_log1p_moments_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
+int rsc_normalize_log1p_moments(rsc_csr* X, float target_sum, const int64_t* cell_total_i64,
+                                const int32_t* gene_n_cells, int which_moments, int ddof,
+                                double* mean_log, double* var_log,
+                                double* mean_lin, double* var_lin, double* gene_sums_out,
+                                void* ws, size_t ws_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------
+ * rsc_moments_finalize — mean_j = S1_j / n, var_j = max(0, (S2_j - n mean_j^2)/(n - ddof))
+ * from raw per-gene sums (the last step of PAPER.md:L91's mean / variance kernel, split
+ * out so that sums from several row shards (L141: chunks along the cell axis) can be
+ * added first).  n_rows_total is the number of cells over ALL shards.
+ * ------------------------------------------------------------------------------- */
+int rsc_moments_finalize(int32_t n_genes, int64_t n_rows_total, int ddof, const double* S1,
+                         const double* S2, double* gene_mean, double* gene_var, void* stream);
+
+/* ---------------------------------------------------------------------------------
+ * rsc_hvg_select — Seurat-flavour highly-variable-gene selection on the device
+ * ("based on per-gene mean and variance"; L39 "gene selection" kernel
+ * that avoids CPU<->GPU transfers; L87 "follow the algorithmic implementations of
+ * scanpy"; steps H1..H7 of DESIGN.md §3):
+ *   mean==0 -> 1e-12; d = var/mean; [flags bit0] d==0 -> NaN, d = ln d, m = log1p(mean);
+ *   n_bins equal-width right-closed bins over m (first edge lowered by 0.1 % of the
+ *   range); z = (d - mean_bin(d)) / sd_bin(d) (ddof 1, NaNs skipped; a bin with one
+ *   valid gene gives z = 1); cutoff = n_top-th largest non-NaN z; mask = z >= cutoff.
+ *   Outputs (all optional except out_mask / out_count):
+ *     out_mean_t, out_disp, out_disp_norm  double[n_genes]   m, d, z
+ *     out_bin      int32[n_genes]
+ *     out_mask     uint8[n_genes]          1 = selected
+ *     out_indices  int32[n_genes]          selected genes, ascending; tail untouched
+ *     out_count    int32[1]                number selected (>= n_top on ties; the number
+ *                                          of non-NaN genes if that is smaller)
+ *   1 <= n_bins <= 4096, n_top >= 1, n_genes >= 1.
+ * ------------------------------------------------------------------------------- */
+#define RSC_HVG_SEURAT_LOG 1
+size_t rsc_hvg_select_workspace_bytes(int32_t n_genes, int32_t n_bins);
+int rsc_hvg_select(int32_t n_genes, const double* gene_mean, const double* gene_var,
+                   int32_t n_top, int32_t n_bins, int flags,
+                   double* out_mean_t, double* out_disp, double* out_disp_norm,
+                   int32_t* out_bin, uint8_t* out_mask, int32_t* out_indices,
+                   int32_t* out_count, void* ws, size_t ws_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------
+ * rsc_preprocess — the whole chain in one call on device-resident data:
+ * rsc_qc_metrics -> rsc_normalize_log1p_moments -> rsc_hvg_select (fed with the
+ * linear-scale moments when hvg_on_linear != 0, else the log-scale ones; DESIGN.md
+ * reading R8).  `out` collects the device output pointers; see rsc_outputs.
+ * ------------------------------------------------------------------------------- */
+typedef struct {
+  /* per cell [n_rows] */
+  int64_t* cell_total_i64; float* cell_total_f32; int32_t* cell_n_genes;
+  int64_t* cell_flag_total_i64; float* cell_flag_pct;
+  /* per gene [n_cols] */
+  int32_t* gene_n_cells; int64_t* gene_total_i64;
+  double* mean_log; double* var_log; double* mean_lin; double* var_lin;
+  double* hvg_mean_t; double* hvg_disp; double* hvg_disp_norm; int32_t* hvg_bin;
+  uint8_t* hvg_mask; int32_t* hvg_indices;
+  int32_t* hvg_count; /* [1] */
+} rsc_outputs;
+
+typedef struct {
+  float target_sum;
+  int32_t n_top;
+  int32_t n_bins;
+  int32_t ddof;
+  int32_t which_moments;  /* RSC_MOMENTS_* bits                                */
+  int32_t hvg_on_linear;  /* 1: HVG consumes linear-scale moments, 0: log-scale */
+  int32_t hvg_flags;      /* RSC_HVG_* bits                                     */
+} rsc_params;
+
+size_t rsc_preprocess_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz, int32_t n_bins);
+int rsc_preprocess(rsc_csr* X, const uint8_t* gene_flags, const rsc_params* prm,
+                   const rsc_outputs* out, void* ws, size_t ws_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------
+ * rsc_preprocess_host — the same chain for a matrix that lives in HOST memory
+ * ("a single function transfers data to GPU memory").  `host_X` holds
+ * HOST pointers (pinned memory recommended), `host_out` HOST output pointers (any may
+ * be NULL); `host_data_out` optionally receives the log-normalised values.  The call
+ * stages everything through the caller's device workspace `dev_ws` (size from
+ * rsc_preprocess_host_workspace_bytes), enqueues H2D copies, the chain and D2H copies
+ * on `stream`, and returns without synchronising; the caller synchronises the stream
+ * before reading the host outputs.
+ * ------------------------------------------------------------------------------- */
+size_t rsc_preprocess_host_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz, int32_t n_bins);
+int rsc_preprocess_host(const rsc_csr* host_X, const uint8_t* host_gene_flags,
+                        const rsc_params* prm, const rsc_outputs* host_out,
+                        float* host_data_out, void* dev_ws, size_t dev_ws_bytes, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RSC_H_ */

@@ -1,0 +1,257 @@
+// C ABI of librsc_b200 (include/rsc.h): host-side argument validation, workspace carving,
+// dispatch between the sorted-row shared-memory kernels and the generic L2-atomic kernels,
+// and the two whole-chain entry points.  No device allocation, no stream synchronisation.
+#include <math.h>
+#include <stdarg.h>
+#include <string.h>
+
+#include "common.cuh"
+
+namespace rsc {
+
+static thread_local char g_err[512] = "";
+unsigned long long g_launch_count = 0;
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+static int g_dev_checked = -1;   // device ordinal whose capability was verified
+static int g_sm_count = kNumSMs;
+
+int check_device() {
+  int dev = -1;
+  RSC_CUDA(cudaGetDevice(&dev));
+  if (dev == g_dev_checked) return RSC_OK;
+  int major = 0, sms = 0;
+  RSC_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+  RSC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  if (major != 10) {
+    set_error("device %d has compute capability %d.x; librsc_b200 is built for sm_100a only", dev,
+              major);
+    return RSC_ERR_UNSUPPORTED;
+  }
+  g_sm_count = sms;
+  g_dev_checked = dev;
+  return RSC_OK;
+}
+
+int sm_count() { return g_sm_count; }
+
+static int check_csr(const rsc_csr* X, const char* who, bool need_data) {
+  RSC_CHECK_ARG(X != nullptr, "%s: X is NULL", who);
+  RSC_CHECK_ARG(X->n_rows >= 0, "%s: n_rows < 0", who);
+  RSC_CHECK_ARG(X->n_cols > 0, "%s: n_cols <= 0", who);
+  RSC_CHECK_ARG(X->nnz >= 0, "%s: nnz < 0", who);
+  RSC_CHECK_ARG(X->indptr != nullptr, "%s: indptr is NULL", who);
+  RSC_CHECK_ARG(X->nnz == 0 || X->indices != nullptr, "%s: indices is NULL", who);
+  RSC_CHECK_ARG(X->nnz == 0 || !need_data || X->data != nullptr, "%s: data is NULL", who);
+  return RSC_OK;
+}
+
+static int check_ws(const char* who, void* ws, size_t have, size_t need) {
+  if (need == 0) return RSC_OK;
+  if (ws == nullptr || have < need || (reinterpret_cast<uintptr_t>(ws) & 255)) {
+    set_error("%s: workspace too small or misaligned (have %zu, need %zu, 256-byte aligned)", who,
+              have, need);
+    return RSC_ERR_WORKSPACE;
+  }
+  return RSC_OK;
+}
+
+// implemented in generic.cu
+int launch_qc_generic(const rsc_csr&, const uint8_t*, int64_t*, float*, int32_t*, int64_t*, float*,
+                      int32_t*, int64_t*, cudaStream_t);
+int launch_moments_generic(const rsc_csr&, int, double*, double*, cudaStream_t);
+int launch_fused_generic(const rsc_csr&, float, const int64_t*, int, double*, double*, double*,
+                         double*, cudaStream_t);
+int finalize_moments(int32_t, int64_t, int, const double*, const double*, double*, double*,
+                     cudaStream_t);
+
+size_t qc_workspace_bytes(int64_t, int32_t, int64_t) { return 256; }
+size_t moments_workspace_bytes(int64_t, int32_t n_cols, int64_t) {
+  return 2 * align_up(sizeof(double) * (size_t)n_cols, 256);
+}
+size_t fused_workspace_bytes(int64_t, int32_t n_cols, int64_t) {
+  return 4 * align_up(sizeof(double) * (size_t)n_cols, 256);
+}
+
+int launch_qc(const rsc_csr& X, const uint8_t* gene_flags, int64_t* cell_total_i64,
+              float* cell_total_f32, int32_t* cell_n_genes, int64_t* cell_flag_total_i64,
+              float* cell_flag_pct, int32_t* gene_n_cells, int64_t* gene_total_i64, void*, size_t,
+              cudaStream_t st) {
+  return launch_qc_generic(X, gene_flags, cell_total_i64, cell_total_f32, cell_n_genes,
+                           cell_flag_total_i64, cell_flag_pct, gene_n_cells, gene_total_i64, st);
+}
+
+int launch_moments(const rsc_csr& X, int transform, int ddof, double* mean, double* var,
+                   double* sum, double* sumsq, void* ws, size_t, cudaStream_t st) {
+  const size_t gsz = align_up(sizeof(double) * (size_t)X.n_cols, 256);
+  unsigned char* w = static_cast<unsigned char*>(ws);
+  double* S1 = sum ? sum : reinterpret_cast<double*>(w);
+  double* S2 = sumsq ? sumsq : reinterpret_cast<double*>(w + gsz);
+  int rc = launch_moments_generic(X, transform, S1, S2, st);
+  if (rc != RSC_OK) return rc;
+  return finalize_moments(X.n_cols, X.n_rows, ddof, S1, S2, mean, var, st);
+}
+
+int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i64,
+                 const int32_t* /*gene_n_cells*/, int which, int ddof, double* mean_log,
+                 double* var_log, double* mean_lin, double* var_lin, double* sums_out, void* ws,
+                 size_t, cudaStream_t st) {
+  const size_t gsz = align_up(sizeof(double) * (size_t)X.n_cols, 256);
+  unsigned char* w = static_cast<unsigned char*>(ws);
+  const size_t G = (size_t)X.n_cols;
+  double* S1log = sums_out ? sums_out : reinterpret_cast<double*>(w);
+  double* S2log = sums_out ? sums_out + G : reinterpret_cast<double*>(w + gsz);
+  double* S1lin = sums_out ? sums_out + 2 * G : reinterpret_cast<double*>(w + 2 * gsz);
+  double* S2lin = sums_out ? sums_out + 3 * G : reinterpret_cast<double*>(w + 3 * gsz);
+  int rc = launch_fused_generic(X, target_sum, cell_total_i64, which, S1log, S2log, S1lin, S2lin, st);
+  if (rc != RSC_OK) return rc;
+  if (which & RSC_MOMENTS_LOG) {
+    rc = finalize_moments(X.n_cols, X.n_rows, ddof, S1log, S2log, mean_log, var_log, st);
+    if (rc != RSC_OK) return rc;
+  }
+  if (which & RSC_MOMENTS_LIN) {
+    rc = finalize_moments(X.n_cols, X.n_rows, ddof, S1lin, S2lin, mean_lin, var_lin, st);
+    if (rc != RSC_OK) return rc;
+  }
+  return RSC_OK;
+}
+
+}  // namespace rsc
+
+using namespace rsc;
+
+extern "C" {
+
+const char* rsc_last_error(void) { return g_err; }
+const char* rsc_version(void) { return "0.1.0"; }
+uint64_t rsc_kernel_launch_count(void) { return g_launch_count; }
+
+size_t rsc_qc_metrics_workspace_bytes(int64_t n, int32_t G, int64_t nnz) {
+  return qc_workspace_bytes(n, G, nnz);
+}
+
+int rsc_qc_metrics(const rsc_csr* X, const uint8_t* gene_flags, int64_t* cell_total_i64,
+                   float* cell_total_f32, int32_t* cell_n_genes, int64_t* cell_flag_total_i64,
+                   float* cell_flag_pct, int32_t* gene_n_cells, int64_t* gene_total_i64, void* ws,
+                   size_t ws_bytes, void* stream) {
+  int rc = check_csr(X, "rsc_qc_metrics", true);
+  if (rc) return rc;
+  if ((rc = check_device())) return rc;
+  if ((rc = check_ws("rsc_qc_metrics", ws, ws_bytes, qc_workspace_bytes(X->n_rows, X->n_cols, X->nnz))))
+    return rc;
+  return launch_qc(*X, gene_flags, cell_total_i64, cell_total_f32, cell_n_genes,
+                   cell_flag_total_i64, cell_flag_pct, gene_n_cells, gene_total_i64, ws, ws_bytes,
+                   static_cast<cudaStream_t>(stream));
+}
+
+int rsc_normalize_total(rsc_csr* X, float target_sum, const int64_t* cell_total_i64,
+                        float* cell_scale_out, void* stream) {
+  int rc = check_csr(X, "rsc_normalize_total", true);
+  if (rc) return rc;
+  RSC_CHECK_ARG(isfinite(target_sum) && target_sum > 0.0f,
+                "rsc_normalize_total: target_sum must be finite and > 0");
+  if ((rc = check_device())) return rc;
+  return launch_normalize(*X, target_sum, cell_total_i64, cell_scale_out,
+                          static_cast<cudaStream_t>(stream));
+}
+
+int rsc_log1p(rsc_csr* X, void* stream) {
+  int rc = check_csr(X, "rsc_log1p", true);
+  if (rc) return rc;
+  if ((rc = check_device())) return rc;
+  return launch_log1p(*X, static_cast<cudaStream_t>(stream));
+}
+
+size_t rsc_gene_moments_workspace_bytes(int64_t n, int32_t G, int64_t nnz) {
+  return moments_workspace_bytes(n, G, nnz);
+}
+
+int rsc_gene_moments(const rsc_csr* X, int transform, int ddof, double* gene_mean,
+                     double* gene_var, double* gene_sum, double* gene_sumsq, void* ws,
+                     size_t ws_bytes, void* stream) {
+  int rc = check_csr(X, "rsc_gene_moments", true);
+  if (rc) return rc;
+  RSC_CHECK_ARG(transform == 0 || transform == 1, "rsc_gene_moments: transform must be 0 or 1");
+  RSC_CHECK_ARG(ddof == 0 || ddof == 1, "rsc_gene_moments: ddof must be 0 or 1");
+  RSC_CHECK_ARG(X->n_rows - ddof > 0, "rsc_gene_moments: n_rows - ddof must be > 0");
+  RSC_CHECK_ARG(gene_mean != nullptr && gene_var != nullptr,
+                "rsc_gene_moments: gene_mean / gene_var are required");
+  if ((rc = check_device())) return rc;
+  if ((rc = check_ws("rsc_gene_moments", ws, ws_bytes,
+                     moments_workspace_bytes(X->n_rows, X->n_cols, X->nnz))))
+    return rc;
+  return launch_moments(*X, transform, ddof, gene_mean, gene_var, gene_sum, gene_sumsq, ws,
+                        ws_bytes, static_cast<cudaStream_t>(stream));
+}
+
+size_t rsc_normalize_log1p_moments_workspace_bytes(int64_t n, int32_t G, int64_t nnz) {
+  return fused_workspace_bytes(n, G, nnz);
+}
+
+int rsc_normalize_log1p_moments(rsc_csr* X, float target_sum, const int64_t* cell_total_i64,
+                                const int32_t* gene_n_cells, int which_moments, int ddof,
+                                double* mean_log, double* var_log, double* mean_lin,
+                                double* var_lin, double* gene_sums_out, void* ws, size_t ws_bytes,
+                                void* stream) {
+  int rc = check_csr(X, "rsc_normalize_log1p_moments", true);
+  if (rc) return rc;
+  RSC_CHECK_ARG(isfinite(target_sum) && target_sum > 0.0f,
+                "rsc_normalize_log1p_moments: target_sum must be finite and > 0");
+  RSC_CHECK_ARG(cell_total_i64 != nullptr, "rsc_normalize_log1p_moments: cell_total_i64 is required");
+  RSC_CHECK_ARG((which_moments & ~3) == 0, "rsc_normalize_log1p_moments: bad which_moments");
+  RSC_CHECK_ARG(ddof == 0 || ddof == 1, "rsc_normalize_log1p_moments: ddof must be 0 or 1");
+  RSC_CHECK_ARG(which_moments == 0 || X->n_rows - ddof > 0,
+                "rsc_normalize_log1p_moments: n_rows - ddof must be > 0");
+  RSC_CHECK_ARG(!(which_moments & RSC_MOMENTS_LOG) || (mean_log && var_log),
+                "rsc_normalize_log1p_moments: mean_log / var_log required with RSC_MOMENTS_LOG");
+  RSC_CHECK_ARG(!(which_moments & RSC_MOMENTS_LIN) || (mean_lin && var_lin),
+                "rsc_normalize_log1p_moments: mean_lin / var_lin required with RSC_MOMENTS_LIN");
+  if ((rc = check_device())) return rc;
+  if ((rc = check_ws("rsc_normalize_log1p_moments", ws, ws_bytes,
+                     fused_workspace_bytes(X->n_rows, X->n_cols, X->nnz))))
+    return rc;
+  return launch_fused(*X, target_sum, cell_total_i64, gene_n_cells, which_moments, ddof, mean_log,
+                      var_log, mean_lin, var_lin, gene_sums_out, ws, ws_bytes,
+                      static_cast<cudaStream_t>(stream));
+}
+
+int rsc_moments_finalize(int32_t n_genes, int64_t n_rows_total, int ddof, const double* S1,
+                         const double* S2, double* gene_mean, double* gene_var, void* stream) {
+  RSC_CHECK_ARG(n_genes >= 1, "rsc_moments_finalize: n_genes < 1");
+  RSC_CHECK_ARG(S1 && S2 && gene_mean && gene_var, "rsc_moments_finalize: NULL pointer");
+  RSC_CHECK_ARG(ddof == 0 || ddof == 1, "rsc_moments_finalize: ddof must be 0 or 1");
+  RSC_CHECK_ARG(n_rows_total - ddof > 0, "rsc_moments_finalize: n_rows_total - ddof must be > 0");
+  int rc = check_device();
+  if (rc) return rc;
+  return finalize_moments(n_genes, n_rows_total, ddof, S1, S2, gene_mean, gene_var,
+                          static_cast<cudaStream_t>(stream));
+}
+
+size_t rsc_hvg_select_workspace_bytes(int32_t G, int32_t n_bins) {
+  return hvg_workspace_bytes(G, n_bins);
+}
+
+int rsc_hvg_select(int32_t n_genes, const double* gene_mean, const double* gene_var, int32_t n_top,
+                   int32_t n_bins, int flags, double* out_mean_t, double* out_disp,
+                   double* out_disp_norm, int32_t* out_bin, uint8_t* out_mask,
+                   int32_t* out_indices, int32_t* out_count, void* ws, size_t ws_bytes,
+                   void* stream) {
+  RSC_CHECK_ARG(n_genes >= 1, "rsc_hvg_select: n_genes < 1");
+  RSC_CHECK_ARG(gene_mean && gene_var, "rsc_hvg_select: gene_mean / gene_var are required");
+  RSC_CHECK_ARG(n_top >= 1, "rsc_hvg_select: n_top < 1");
+  RSC_CHECK_ARG(n_bins >= 1 && n_bins <= 4096, "rsc_hvg_select: n_bins must be in [1, 4096]");
+  RSC_CHECK_ARG(out_mask && out_count, "rsc_hvg_select: out_mask / out_count are required");
+  int rc = check_device();
+  if (rc) return rc;
+  return launch_hvg(n_genes, gene_mean, gene_var, n_top, n_bins, flags, out_mean_t, out_disp,
+                    out_disp_norm, out_bin, out_mask, out_indices, out_count, ws, ws_bytes,
+                    static_cast<cudaStream_t>(stream));
+}
+
+}  // extern "C"

@@ -1,0 +1,103 @@
+// Shared host/device helpers of librsc_b200 (CUDA path only; the CPU oracle shares nothing
+// with this tree).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "rsc.h"
+
+namespace rsc {
+
+constexpr int kNumSMs = 148;       // B200: 2 dies x 74 SMs (grid sizing)
+constexpr int kWarp = 32;
+
+void set_error(const char* fmt, ...);
+
+#define RSC_CHECK_ARG(cond, ...)                 \
+  do {                                           \
+    if (!(cond)) {                               \
+      ::rsc::set_error(__VA_ARGS__);             \
+      return RSC_ERR_INVALID_ARG;                \
+    }                                            \
+  } while (0)
+
+#define RSC_CUDA(call)                                                              \
+  do {                                                                              \
+    cudaError_t e__ = (call);                                                       \
+    if (e__ != cudaSuccess) {                                                       \
+      ::rsc::set_error("%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__),     \
+                       __FILE__, __LINE__);                                         \
+      return RSC_ERR_CUDA;                                                          \
+    }                                                                               \
+  } while (0)
+
+extern unsigned long long g_launch_count;   // kernels launched by this library (host counter)
+
+#define RSC_LAUNCH_CHECK(name)                                                      \
+  do {                                                                              \
+    ++::rsc::g_launch_count;                                                        \
+    cudaError_t e__ = cudaGetLastError();                                           \
+    if (e__ != cudaSuccess) {                                                       \
+      ::rsc::set_error("launch of %s failed: %s", name, cudaGetErrorString(e__));   \
+      return RSC_ERR_CUDA;                                                          \
+    }                                                                               \
+  } while (0)
+
+// Returns RSC_OK when the current device is compute capability 10.x.
+int check_device();
+// Number of SMs of the current device (148 on B200).
+int sm_count();
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ---- launchers implemented in the kernel translation units -------------------------
+int launch_qc(const rsc_csr& X, const uint8_t* gene_flags, int64_t* cell_total_i64,
+              float* cell_total_f32, int32_t* cell_n_genes, int64_t* cell_flag_total_i64,
+              float* cell_flag_pct, int32_t* gene_n_cells, int64_t* gene_total_i64, void* ws,
+              size_t ws_bytes, cudaStream_t st);
+size_t qc_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
+
+int launch_normalize(const rsc_csr& X, float target_sum, const int64_t* cell_total_i64,
+                     float* cell_scale_out, cudaStream_t st);
+int launch_log1p(const rsc_csr& X, cudaStream_t st);
+
+// mode: 0 = plain moments of data (transform 0/1), 1 = fused normalise+log1p+moments.
+int launch_moments(const rsc_csr& X, int transform, int ddof, double* mean, double* var,
+                   double* sum, double* sumsq, void* ws, size_t ws_bytes, cudaStream_t st);
+size_t moments_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
+
+int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i64,
+                 const int32_t* gene_n_cells, int which, int ddof, double* mean_log,
+                 double* var_log, double* mean_lin, double* var_lin, double* sums_out, void* ws,
+                 size_t ws_bytes, cudaStream_t st);
+int finalize_moments(int32_t G, int64_t n, int ddof, const double* S1, const double* S2,
+                     double* mean, double* var, cudaStream_t st);
+size_t fused_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
+
+int launch_hvg(int32_t G, const double* mean, const double* var, int32_t n_top, int32_t n_bins,
+               int flags, double* out_mean_t, double* out_disp, double* out_disp_norm,
+               int32_t* out_bin, uint8_t* out_mask, int32_t* out_indices, int32_t* out_count,
+               void* ws, size_t ws_bytes, cudaStream_t st);
+size_t hvg_workspace_bytes(int32_t G, int32_t n_bins);
+
+// ---- device helpers ----------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
+
+template <typename T>
+__device__ __forceinline__ T warp_sum(T v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// scale_i of normalize_total: one float32 division, shared by the unfused and the fused
+// kernels so that their x' are bit-identical (reading R5).
+__device__ __forceinline__ float cell_scale(float target_sum, int64_t total) {
+  return total != 0 ? __fdiv_rn(target_sum, (float)total) : 1.0f;
+}
+#endif
+
+}  // namespace rsc

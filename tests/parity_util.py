@@ -1,0 +1,119 @@
+"""Helpers shared by the GPU parity tests: upload / download, sub-matrix extraction (torch
+indexing only — plumbing, no method arithmetic) and the tolerance checks stated in
+BASELINE.json's north_star and derived in DESIGN.md §6."""
+import numpy as np
+import torch
+
+RTOL_F32 = 1e-5       # float32 values (north_star; PAPER.md:L155 allclose rtol)
+RTOL_MOM = 1e-9       # fp64-accumulated gene moments (north_star)
+
+
+def to_dev(indptr, indices, data, G, sorted_indices=True):
+    from paper_2603_02402_b200 import Csr
+    return Csr(torch.as_tensor(np.asarray(indptr, np.int64)).cuda(),
+               torch.as_tensor(np.asarray(indices, np.int32)).cuda(),
+               torch.as_tensor(np.asarray(data, np.float32)).cuda(), G, sorted_indices)
+
+
+def clone(X):
+    from paper_2603_02402_b200 import Csr
+    return Csr(X.indptr, X.indices, X.data.clone(), X.n_cols, X.sorted_indices)
+
+
+def np_(t):
+    return t.detach().cpu().numpy()
+
+
+def assert_int_equal(got, want, name):
+    got = np_(got) if isinstance(got, torch.Tensor) else got
+    assert got.dtype == want.dtype, f"{name}: dtype {got.dtype} vs {want.dtype}"
+    assert np.array_equal(got, want), f"{name}: integer output differs"
+
+
+def assert_f32_close(got, want, name, rtol=RTOL_F32):
+    got = np_(got) if isinstance(got, torch.Tensor) else got
+    got = got.astype(np.float64); want = np.asarray(want, np.float64)
+    assert np.array_equal(np.isnan(got), np.isnan(want)), f"{name}: NaN pattern differs"
+    ok = ~np.isnan(want)
+    err = np.abs(got[ok] - want[ok])
+    assert np.all(err <= rtol * np.abs(want[ok])), \
+        f"{name}: max rel err {np.max(err / np.maximum(np.abs(want[ok]), 1e-300)):.3e}"
+
+
+def assert_moments_close(mean_g, var_g, mean_o, var_o, name):
+    """mean: rtol 1e-9.  var: rtol 1e-9 plus the rounding floor of the one-pass formula
+    (S2 - n mean^2)/(n - ddof), 64 eps * mean^2."""
+    mean_g = np_(mean_g) if isinstance(mean_g, torch.Tensor) else mean_g
+    var_g = np_(var_g) if isinstance(var_g, torch.Tensor) else var_g
+    em = np.abs(mean_g - mean_o)
+    assert np.all(em <= RTOL_MOM * np.abs(mean_o)), f"{name}: mean rel err {np.max(em / np.maximum(np.abs(mean_o), 1e-300)):.3e}"
+    ev = np.abs(var_g - var_o)
+    tol = RTOL_MOM * np.abs(var_o) + 64 * 2.2e-16 * mean_o * mean_o
+    assert np.all(ev <= tol), f"{name}: var err, worst ratio {np.max(ev / np.maximum(tol, 1e-300)):.3e}"
+
+
+def assert_hvg_matches(g, o, n_top, name, strict=True):
+    """g: GPU outputs (dict of tensors), o: oracle dict computed from the SAME mean / var."""
+    gm, gd, gz = np_(g["mean_t"]), np_(g["disp"]), np_(g["disp_norm"])
+    assert np.array_equal(np.isnan(gd), np.isnan(o["disp"])), f"{name}: disp NaN pattern"
+    ok = ~np.isnan(o["disp"])
+    np.testing.assert_allclose(gm, o["mean_t"], rtol=1e-12, atol=1e-300, err_msg=name)
+    np.testing.assert_allclose(gd[ok], o["disp"][ok], rtol=1e-12, atol=1e-13, err_msg=name)
+    gb = np_(g["bin"])
+    nb_diff = int(np.sum(gb != o["bin"]))
+    # libm ulp differences in log1p can move a gene sitting exactly on an edge
+    assert nb_diff <= (0 if strict else 2), f"{name}: {nb_diff} bin ids differ"
+    if nb_diff == 0:
+        assert np.array_equal(np.isnan(gz), np.isnan(o["disp_norm"])), f"{name}: z NaN pattern"
+        okz = ~np.isnan(o["disp_norm"])
+        np.testing.assert_allclose(gz[okz], o["disp_norm"][okz], rtol=1e-9, atol=1e-10, err_msg=name)
+    mask_g = np_(g["mask"]).astype(bool)
+    mask_o = o["mask"].astype(bool)
+    cnt = int(np_(g["count"])[0])
+    assert cnt == int(mask_g.sum()), f"{name}: count {cnt} != popcount(mask) {mask_g.sum()}"
+    idx = np_(g["indices"])[:cnt]
+    assert np.array_equal(idx, np.nonzero(mask_g)[0]), f"{name}: indices not the ascending mask positions"
+    if not np.array_equal(mask_g, mask_o):
+        # identical except for ties at the cutoff (north_star; reading R13)
+        cutoff = o["cutoff"]
+        band = 1e-9 * max(1.0, abs(cutoff))
+        diff = np.nonzero(mask_g != mask_o)[0]
+        zz = o["disp_norm"][diff]
+        assert np.all(np.abs(zz - cutoff) <= band), f"{name}: HVG sets differ outside the tie band"
+    valid = int((~np.isnan(o["disp_norm"])).sum())
+    assert cnt >= min(n_top, valid)
+
+
+def extract_rows(indptr, indices, data_list, rows):
+    """Sub-CSR holding the given rows (device tensors in, numpy out)."""
+    rows = torch.as_tensor(rows, device=indptr.device, dtype=torch.int64)
+    beg = indptr[rows]; end = indptr[rows + 1]
+    ln = end - beg
+    ip = torch.zeros(rows.numel() + 1, dtype=torch.int64, device=indptr.device)
+    torch.cumsum(ln, 0, out=ip[1:])
+    tot = int(ip[-1])
+    rid = torch.repeat_interleave(torch.arange(rows.numel(), device=indptr.device), ln)
+    pos = beg[rid] + (torch.arange(tot, device=indptr.device) - ip[rid])
+    return np_(ip), np_(indices[pos]), [np_(d[pos]) for d in data_list], pos
+
+
+def extract_cols(indptr, indices, data_list, cols, n_cols, chunk=1 << 28):
+    """Sub-CSR (all rows) restricted to the given columns, columns renumbered 0..len(cols)-1."""
+    dev = indptr.device
+    cols = torch.as_tensor(cols, device=dev, dtype=torch.int64)
+    lut = torch.full((n_cols,), -1, dtype=torch.int32, device=dev)
+    lut[cols] = torch.arange(cols.numel(), dtype=torch.int32, device=dev)
+    nnz = indices.numel()
+    pos_parts = []
+    for s in range(0, nnz, chunk):
+        e = min(nnz, s + chunk)
+        m = lut[indices[s:e].long()] >= 0
+        pos_parts.append(torch.nonzero(m).squeeze(1) + s)
+        del m
+    pos = torch.cat(pos_parts) if pos_parts else torch.zeros(0, dtype=torch.int64, device=dev)
+    n = indptr.numel() - 1
+    rid = torch.searchsorted(indptr, pos, right=True) - 1
+    cnt = torch.bincount(rid, minlength=n)
+    ip = torch.zeros(n + 1, dtype=torch.int64, device=dev)
+    torch.cumsum(cnt, 0, out=ip[1:])
+    return np_(ip), np_(lut[indices[pos].long()]), [np_(d[pos]) for d in data_list]

@@ -1,0 +1,172 @@
+"""GPU parity on BASELINE.json's configurations, through rsc_preprocess (the call bench.py
+times) and rsc_preprocess_host.
+
+Config 1 is checked element by element against the full oracle chain.  The large configs are
+checked at FULL size in the bench launch configuration on sampled outputs the oracle computes
+one by one (sampled rows for per-cell outputs and x''; sampled genes for per-gene outputs),
+plus invariants that hold at any size and the HVG selection recomputed by the oracle from the
+GPU's full mean / var arrays.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle_np as O
+from paper_2603_02402_b200 import synth
+import parity_util as U
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _lib():
+    from paper_2603_02402_b200 import build, binding
+    build.build()
+    binding.lib()
+
+
+def _run_chain(cfg, X, flags, which=3, hvg_on_linear=True):
+    from paper_2603_02402_b200 import Preprocessor
+    pp = Preprocessor(X.n_rows, X.n_cols, X.nnz, cfg.target_sum, cfg.n_top, cfg.n_bins, 1, which,
+                      hvg_on_linear)
+    out = pp.run(X, flags)
+    torch.cuda.synchronize()
+    return out
+
+
+def test_config1_full_oracle():
+    from paper_2603_02402_b200 import Csr
+    cfg = synth.CONFIGS[1]
+    indptr, indices, data = synth.make_csr(cfg, "cuda")
+    flags = synth.gene_flags(cfg, "cuda")
+    raw = data.clone()
+    X = Csr(indptr, indices, data, cfg.n_genes)
+    out = _run_chain(cfg, X, flags)
+    ip, ix, rw = U.np_(indptr), U.np_(indices), U.np_(raw)
+    ref = O.preprocess_chain(ip, ix, rw, cfg.n_genes, U.np_(flags), cfg.target_sum, cfg.n_top, cfg.n_bins)
+    for k in ("cell_total_i64", "cell_n_genes", "cell_flag_total_i64", "gene_n_cells", "gene_total_i64"):
+        U.assert_int_equal(out[k], ref["qc"][k], k)
+    U.assert_f32_close(out["cell_flag_pct"], ref["qc"]["cell_flag_pct"], "pct")
+    U.assert_f32_close(X.data, ref["x_log"], "x''")
+    xl = U.np_(X.data)
+    mo, vo, _, _ = O.gene_moments(ip, ix, xl, cfg.n_genes)
+    U.assert_moments_close(out["mean_log"], out["var_log"], mo, vo, "log moments")
+    np.testing.assert_allclose(U.np_(out["mean_lin"]), ref["mean_lin"], rtol=1e-6)
+    np.testing.assert_allclose(U.np_(out["var_lin"]), ref["var_lin"], rtol=1e-6)
+    # HVG: oracle fed with the GPU's own fp64 moments -> identical set
+    h = O.hvg_select(U.np_(out["mean_lin"]), U.np_(out["var_lin"]), cfg.n_top, cfg.n_bins)
+    g = dict(mean_t=out["hvg_mean_t"], disp=out["hvg_disp"], disp_norm=out["hvg_disp_norm"],
+             bin=out["hvg_bin"], mask=out["hvg_mask"], indices=out["hvg_indices"], count=out["hvg_count"])
+    U.assert_hvg_matches(g, h, cfg.n_top, "cfg1 hvg", strict=False)
+    # independent chains: the sets agree except near the cutoff
+    m_o = ref["hvg"]["mask"].astype(bool); m_g = U.np_(out["hvg_mask"]).astype(bool)
+    assert (m_o != m_g).sum() <= 4
+
+
+def _sampled_check(cfg, n_cells=None, n_row_samples=384, n_gene_samples=64):
+    from paper_2603_02402_b200 import Csr, rsc_normalize_total
+    n = cfg.n_cells if n_cells is None else n_cells
+    indptr, indices, data = synth.make_csr(cfg, "cuda", n_cells=n)
+    G = cfg.n_genes
+    nnz = indices.numel()
+    flags = synth.gene_flags(cfg, "cuda")
+    raw = data.clone()
+    X = Csr(indptr, indices, data, G)
+    out = _run_chain(cfg, X, flags)
+
+    # invariants at any size
+    assert int(indptr[-1]) == nnz
+    assert int(out["gene_n_cells"].sum(dtype=torch.int64)) == nnz == int(out["cell_n_genes"].sum(dtype=torch.int64))
+    assert int(out["gene_total_i64"].sum()) == int(out["cell_total_i64"].sum())
+    assert torch.equal(out["cell_n_genes"].long(), indptr[1:] - indptr[:-1])
+    assert bool((X.data > 0).all())
+
+    # sampled rows (+ the longest and the shortest row)
+    rng = np.random.default_rng(cfg.seed)
+    ln = indptr[1:] - indptr[:-1]
+    rows = np.unique(np.concatenate([rng.integers(0, n, n_row_samples),
+                                     [int(ln.argmax()), int(ln.argmin()), 0, n - 1]]))
+    ip, ix, (rw, xl_g), _ = U.extract_rows(indptr, indices, [raw, X.data], rows)
+    q = O.qc_metrics(ip, ix, rw, G, U.np_(flags))
+    rsel = torch.as_tensor(rows).cuda()
+    for k in ("cell_total_i64", "cell_n_genes", "cell_flag_total_i64"):
+        U.assert_int_equal(out[k][rsel], q[k], k)
+    U.assert_f32_close(out["cell_flag_pct"][rsel], q["cell_flag_pct"], "pct")
+    xl_o = O.log1p(O.normalize_total(ip, rw, cfg.target_sum, q["cell_total_i64"])[0])
+    U.assert_f32_close(xl_g, xl_o, "x'' sampled rows")
+
+    # sampled genes (+ flagged ones and the most / least detected)
+    nc = out["gene_n_cells"]
+    genes = np.unique(np.concatenate([rng.integers(0, G, n_gene_samples), np.arange(4),
+                                      [int(nc.argmax()), int(nc.argmin())]]))
+    Xn = Csr(indptr, indices, raw.clone(), G)
+    rsc_normalize_total(Xn, cfg.target_sum, out["cell_total_i64"])
+    ipc, ixc, (rwc, xlc, xnc) = U.extract_cols(indptr, indices, [raw, X.data, Xn.data], genes, G)
+    del Xn
+    k = len(genes)
+    qg = O.qc_metrics(ipc, ixc, rwc, k, None)
+    gsel = torch.as_tensor(genes).cuda()
+    U.assert_int_equal(out["gene_n_cells"][gsel], qg["gene_n_cells"], "gene_n_cells")
+    U.assert_int_equal(out["gene_total_i64"][gsel], qg["gene_total_i64"], "gene_total_i64")
+    mo, vo, _, _ = O.gene_moments(ipc, ixc, xlc, k)
+    U.assert_moments_close(out["mean_log"][gsel], out["var_log"][gsel], mo, vo, "log moments (sampled genes)")
+    mo, vo, _, _ = O.gene_moments(ipc, ixc, xnc, k)
+    U.assert_moments_close(out["mean_lin"][gsel], out["var_lin"][gsel], mo, vo, "lin moments (sampled genes)")
+
+    # HVG on the GPU's full moment arrays
+    h = O.hvg_select(U.np_(out["mean_lin"]), U.np_(out["var_lin"]), cfg.n_top, cfg.n_bins)
+    g = dict(mean_t=out["hvg_mean_t"], disp=out["hvg_disp"], disp_norm=out["hvg_disp_norm"],
+             bin=out["hvg_bin"], mask=out["hvg_mask"], indices=out["hvg_indices"], count=out["hvg_count"])
+    U.assert_hvg_matches(g, h, cfg.n_top, f"{cfg.name} hvg", strict=False)
+    return nnz
+
+
+def test_config2_full_size_sampled():
+    nnz = _sampled_check(synth.CONFIGS[2])
+    assert 1.8e8 < nnz < 2.3e8
+
+
+def test_config3_full_size_sampled():
+    nnz = _sampled_check(synth.CONFIGS[3])
+    assert 1.4e9 < nnz < 1.65e9
+
+
+def test_config5_skewed_full_size_sampled():
+    nnz = _sampled_check(synth.CONFIGS[5])
+    assert 1.3e9 < nnz < 1.7e9
+
+
+@pytest.mark.skipif(os.environ.get("RSC_TEST_CFG4", "1") != "1", reason="disabled by RSC_TEST_CFG4")
+def test_config4_int64_nnz_sampled():
+    """7.5e9 nnz (> 2^31): every offset is 64-bit.  ~60 GB matrix + working copies."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 165e9:
+        pytest.skip("needs ~165 GB of free HBM")
+    nnz = _sampled_check(synth.CONFIGS[4], n_row_samples=256, n_gene_samples=32)
+    assert nnz > 2**31
+
+
+def test_host_entry_point_matches_device_chain():
+    from paper_2603_02402_b200 import Csr, HostPreprocessor
+    cfg = synth.CONFIGS[1]
+    indptr, indices, data = synth.make_csr(cfg, "cuda", n_cells=1200)
+    flags = synth.gene_flags(cfg, "cuda")
+    hX = Csr(indptr.cpu().pin_memory(), indices.cpu().pin_memory(), data.cpu().pin_memory(), cfg.n_genes)
+    hp = HostPreprocessor(hX.n_rows, cfg.n_genes, hX.nnz, cfg.target_sum, cfg.n_top, cfg.n_bins,
+                          copy_back_data=True)
+    hout = hp.run(hX, flags.cpu())
+    torch.cuda.synchronize()
+    X = Csr(indptr, indices, data, cfg.n_genes)
+    dout = _run_chain(cfg, X, flags)
+    for k, v in dout.items():
+        a, b = U.np_(v), hout[k].numpy()
+        if k == "hvg_indices":
+            c = int(dout["hvg_count"][0]); a, b = a[:c], b[:c]
+        if a.dtype.kind == "f":
+            np.testing.assert_allclose(b, a, rtol=1e-9, equal_nan=True, err_msg=k)
+        else:
+            assert np.array_equal(a, b), k
+    U.assert_f32_close(hp.data_out, U.np_(X.data), "x'' copied back", rtol=0)
+    assert hp.h2d_bytes == (hX.n_rows + 1) * 8 + hX.nnz * 8 + cfg.n_genes

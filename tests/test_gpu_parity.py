@@ -1,0 +1,238 @@
+"""GPU parity: every C-ABI entry point against the CPU oracle on the same seeded inputs.
+
+Integers bit-exact; float32 values within 1e-5 relative; fp64 moments within 1e-9 when both
+sides read bit-identical float32 inputs; HVG set identical up to ties at the cutoff
+(BASELINE.json north_star).
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle_np as O
+from paper_2603_02402_b200 import synth
+import parity_util as U
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _lib():
+    from paper_2603_02402_b200 import build, binding
+    build.build()
+    binding.lib()
+    assert torch.cuda.is_available()
+
+
+SMALL = [  # n, G, seed, depth, empty_rows, empty_genes  (several tiles + ragged tails + empties)
+    (1, 1, 0, 3.0, (), ()),
+    (3, 7, 1, 2.0, (1,), (2,)),
+    (257, 1031, 2, 0.7, (0, 100, 256), (0, 1030)),
+    (1500, 4099, 3, 0.4, (17,), (5, 6, 7)),
+    (700, 18000, 4, 0.158, (), ()),
+    (33, 36000, 5, 0.6, (32,), ()),
+]
+
+
+def _flags(G, seed):
+    rng = np.random.default_rng(1000 + seed)
+    f = (rng.random(G) < 0.05).astype(np.uint8)
+    f[: min(13, G)] = 1
+    return f
+
+
+def _shuffle_rows_cols(indptr, indices, data, seed):
+    """Same matrix with the entries of every row in random column order (unsorted CSR)."""
+    rng = np.random.default_rng(seed)
+    idx2, dat2 = indices.copy(), data.copy()
+    for i in range(len(indptr) - 1):
+        lo, hi = indptr[i], indptr[i + 1]
+        p = rng.permutation(hi - lo)
+        idx2[lo:hi] = indices[lo:hi][p]; dat2[lo:hi] = data[lo:hi][p]
+    return idx2, dat2
+
+
+@pytest.mark.parametrize("n,G,seed,depth,er,eg", SMALL)
+@pytest.mark.parametrize("sorted_rows", [True, False])
+def test_qc_metrics(n, G, seed, depth, er, eg, sorted_rows):
+    from paper_2603_02402_b200 import rsc_qc_metrics
+    indptr, indices, data, _ = synth.small_nb_csr(n, G, seed, depth, empty_rows=er, empty_genes=eg)
+    if not sorted_rows:
+        indices, data = _shuffle_rows_cols(indptr, indices, data, seed)
+    flags = _flags(G, seed)
+    want = O.qc_metrics(indptr, indices, data, G, flags)
+    X = U.to_dev(indptr, indices, data, G, sorted_rows)
+    got = rsc_qc_metrics(X, torch.as_tensor(flags).cuda())
+    torch.cuda.synchronize()
+    for k in ("cell_total_i64", "cell_n_genes", "cell_flag_total_i64", "gene_n_cells", "gene_total_i64"):
+        U.assert_int_equal(got[k], want[k], k)
+    U.assert_f32_close(got["cell_total_f32"], want["cell_total_f32"], "cell_total_f32", rtol=0)
+    U.assert_f32_close(got["cell_flag_pct"], want["cell_flag_pct"], "cell_flag_pct")
+    # invariants
+    assert int(got["gene_n_cells"].sum()) == int(got["cell_n_genes"].sum()) == len(indices)
+    assert int(got["gene_total_i64"].sum()) == int(got["cell_total_i64"].sum())
+    # no flags -> zero flagged totals
+    got0 = rsc_qc_metrics(X, None)
+    assert int(got0["cell_flag_total_i64"].abs().sum()) == 0
+
+
+@pytest.mark.parametrize("n,G,seed,depth,er,eg", SMALL)
+@pytest.mark.parametrize("s", [1e4, 1e6])
+def test_normalize_then_log1p(n, G, seed, depth, er, eg, s):
+    from paper_2603_02402_b200 import rsc_normalize_total, rsc_log1p, rsc_qc_metrics
+    indptr, indices, data, _ = synth.small_nb_csr(n, G, seed, depth, empty_rows=er, empty_genes=eg)
+    xn_o, scale_o = O.normalize_total(indptr, data, s)
+    xl_o = O.log1p(xn_o)
+    X = U.to_dev(indptr, indices, data, G)
+    scale = rsc_normalize_total(X, s, None, return_scale=True)
+    U.assert_f32_close(X.data, xn_o, "x' (totals summed by the kernel)")
+    U.assert_f32_close(scale, scale_o.astype(np.float32), "scale")
+    # with the exact int64 totals from QC: bit-identical to the self-summed variant
+    X2 = U.to_dev(indptr, indices, data, G)
+    q = rsc_qc_metrics(X2)
+    rsc_normalize_total(X2, s, q["cell_total_i64"])
+    assert torch.equal(X.data, X2.data)
+    # invariant: row sums equal target_sum
+    rows = np.repeat(np.arange(n), np.diff(indptr))
+    rs = np.bincount(rows, weights=U.np_(X.data).astype(np.float64), minlength=n)
+    ne = np.diff(indptr) > 0
+    assert np.all(np.abs(rs[ne] - s) <= s * 1e-6)
+    rsc_log1p(X)
+    U.assert_f32_close(X.data, xl_o, "x''")
+    assert torch.equal(X.indices.cpu(), torch.as_tensor(indices))       # pattern untouched
+    assert np.all((U.np_(X.data) == 0) == (xn_o == 0))
+
+
+def test_log1p_value_range_and_alignment():
+    """Tiny / huge / zero arguments and every 16-byte misalignment of the data pointer."""
+    from paper_2603_02402_b200 import rsc_log1p, Csr
+    vals = np.concatenate([[0.0, 1e-30, 1e-10, 1e-7, 1e-5, 1e-3, 0.02, 0.03, 0.0312, 0.0313, 0.1, 0.5,
+                            1.0, np.e - 1, 10, 1e4, 1e6, 3e7, 1e20],
+                           np.exp(np.random.default_rng(0).uniform(-20, 20, 5000))]).astype(np.float32)
+    want = O.log1p(vals)
+    for off in range(4):
+        for length in (len(vals), 1, 2, 3, 5, 8, 1023):
+            base = torch.zeros(len(vals) + 8, dtype=torch.float32, device="cuda")
+            view = base[off:off + length]
+            view.copy_(torch.as_tensor(vals[:length]))
+            X = Csr(torch.tensor([0, length], dtype=torch.int64, device="cuda"),
+                    torch.zeros(length, dtype=torch.int32, device="cuda"), view, 1)
+            rsc_log1p(X)
+            U.assert_f32_close(view, want[:length], f"log1p off={off} len={length}")
+            assert float(base[:off].abs().sum()) == 0 and float(base[off + length:].abs().sum()) == 0
+
+
+@pytest.mark.parametrize("n,G,seed,depth,er,eg", SMALL[1:])
+@pytest.mark.parametrize("sorted_rows", [True, False])
+def test_gene_moments(n, G, seed, depth, er, eg, sorted_rows):
+    from paper_2603_02402_b200 import rsc_gene_moments
+    indptr, indices, data, _ = synth.small_nb_csr(n, G, seed, depth, empty_rows=er, empty_genes=eg)
+    xl = O.log1p(O.normalize_total(indptr, data, 1e4)[0])
+    if not sorted_rows:
+        indices, xl = _shuffle_rows_cols(indptr, indices, xl, seed)
+    X = U.to_dev(indptr, indices, xl, G, sorted_rows)
+    for transform in (0, 1):
+        for ddof in (1, 0):
+            mo, vo, s1o, s2o = O.gene_moments(indptr, indices, xl, G, transform, ddof)
+            g = rsc_gene_moments(X, transform, ddof)
+            U.assert_moments_close(g["mean"], g["var"], mo, vo, f"moments t={transform} ddof={ddof}")
+            np.testing.assert_allclose(U.np_(g["sum"]), s1o, rtol=1e-12)
+            np.testing.assert_allclose(U.np_(g["sumsq"]), s2o, rtol=1e-12)
+    assert torch.equal(X.data.cpu(), torch.as_tensor(xl))               # read-only
+
+
+@pytest.mark.parametrize("n,G,seed,depth,er,eg", SMALL[1:])
+@pytest.mark.parametrize("s", [1e4, 1e6])
+@pytest.mark.parametrize("which", [1, 2, 3])
+@pytest.mark.parametrize("sorted_rows", [True, False])
+def test_fused_normalize_log1p_moments(n, G, seed, depth, er, eg, s, which, sorted_rows):
+    from paper_2603_02402_b200 import (rsc_normalize_log1p_moments, rsc_normalize_total,
+                                       rsc_qc_metrics)
+    indptr, indices, data, _ = synth.small_nb_csr(n, G, seed, depth, empty_rows=er, empty_genes=eg)
+    if not sorted_rows:
+        indices, data = _shuffle_rows_cols(indptr, indices, data, seed)
+    X = U.to_dev(indptr, indices, data, G, sorted_rows)
+    Xn = U.clone(X)
+    q = rsc_qc_metrics(X)
+    out = rsc_normalize_log1p_moments(X, s, q["cell_total_i64"], q["gene_n_cells"], which, 1)
+    # (a) values against the independent oracle chain
+    xl_o = O.log1p(O.normalize_total(indptr, data, s)[0])
+    U.assert_f32_close(X.data, xl_o, "fused x''")
+    # (b) log-scale moments: oracle M1 on the very x'' the kernel wrote (bit-identical input)
+    if which & 1:
+        mo, vo, _, _ = O.gene_moments(indptr, indices, U.np_(X.data), G, 0, 1)
+        U.assert_moments_close(out["mean_log"], out["var_log"], mo, vo, "fused log moments")
+    # (c) linear-scale moments: oracle M1 on x' written by rsc_normalize_total (same fp32 expr)
+    if which & 2:
+        rsc_normalize_total(Xn, s, q["cell_total_i64"])
+        mo, vo, _, _ = O.gene_moments(indptr, indices, U.np_(Xn.data), G, 0, 1)
+        U.assert_moments_close(out["mean_lin"], out["var_lin"], mo, vo, "fused lin moments")
+    # (d) independent chains end to end at 1e-6
+    if which & 1:
+        mo, vo, _, _ = O.gene_moments(indptr, indices, xl_o, G, 0, 1)
+        np.testing.assert_allclose(U.np_(out["mean_log"]), mo, rtol=1e-6, atol=1e-300)
+        np.testing.assert_allclose(U.np_(out["var_log"]), vo, rtol=1e-6, atol=1e-12)
+
+
+@pytest.mark.parametrize("G,seed,n_top,n_bins", [(1, 0, 1, 20), (2, 1, 1, 20), (50, 2, 5, 20),
+                                                 (1000, 3, 100, 20), (4099, 4, 500, 7),
+                                                 (18000, 5, 2000, 20), (36000, 6, 3000, 20),
+                                                 (30000, 7, 40000, 20), (5000, 8, 1, 1)])
+@pytest.mark.parametrize("log_flag", [1, 0])
+def test_hvg_select_same_inputs(G, seed, n_top, n_bins, log_flag):
+    from paper_2603_02402_b200 import rsc_hvg_select
+    rng = np.random.default_rng(seed)
+    mean = np.exp(rng.normal(-3, 2, G))
+    var = mean * np.exp(rng.normal(0.2, 0.6, G))
+    dead = rng.random(G) < 0.1
+    mean[dead] = 0.0; var[dead] = 0.0                      # undetected genes
+    if G > 10:
+        var[3] = 0.0                                       # zero dispersion -> NaN under the log
+        mean[7] = mean[8]; var[7] = var[8]                 # exact tie
+    o = O.hvg_select(mean, var, n_top, n_bins, seurat_log=bool(log_flag))
+    g = rsc_hvg_select(torch.as_tensor(mean).cuda(), torch.as_tensor(var).cuda(), n_top, n_bins, log_flag)
+    torch.cuda.synchronize()
+    U.assert_hvg_matches(g, o, n_top, f"hvg G={G}", strict=False)
+
+
+def test_hvg_golden_and_degenerate():
+    from paper_2603_02402_b200 import rsc_hvg_select
+    # hand-worked fixture (tests/golden/hvg_tiny.txt, case two_bins / single_gene_bin_and_tie)
+    mean = torch.tensor([1, 2, 3, 4, 5, 6, 7, 8], dtype=torch.float64).cuda()
+    var = torch.tensor([1, 6, 15, 28, 10, 12, 14, 80], dtype=torch.float64).cuda()
+    g = rsc_hvg_select(mean, var, 3, 2, 0)
+    assert U.np_(g["indices"])[:3].tolist() == [2, 3, 7] and int(g["count"][0]) == 3
+    assert U.np_(g["bin"]).tolist() == [0, 0, 0, 0, 1, 1, 1, 1]
+    np.testing.assert_allclose(U.np_(g["disp_norm"])[4:], [-0.5, -0.5, -0.5, 1.5], rtol=1e-14)
+    mean = torch.tensor([1, 2, 3, 10], dtype=torch.float64).cuda()
+    var = torch.tensor([2, 8, 18, 50], dtype=torch.float64).cuda()
+    g = rsc_hvg_select(mean, var, 1, 3, 0)
+    assert int(g["count"][0]) == 2 and U.np_(g["indices"])[:2].tolist() == [2, 3]   # tie at cutoff
+    assert U.np_(g["disp_norm"]).tolist() == [-1.0, 0.0, 1.0, 1.0]
+    # all means equal (reading R10): one bin, still a valid selection
+    mean = np.full(64, 2.5); var = np.linspace(1, 5, 64)
+    o = O.hvg_select(mean, var, 8, 20)
+    g = rsc_hvg_select(torch.as_tensor(mean).cuda(), torch.as_tensor(var).cuda(), 8, 20, 1)
+    U.assert_hvg_matches(g, o, 8, "degenerate")
+    # nothing valid -> empty selection
+    z = torch.zeros(16, dtype=torch.float64).cuda()
+    g = rsc_hvg_select(z, z, 4, 20, 1)
+    assert int(g["count"][0]) == 0 and int(g["mask"].sum()) == 0
+
+
+def test_errors_are_loud():
+    from paper_2603_02402_b200 import binding as B
+    indptr, indices, data, _ = synth.small_nb_csr(10, 20, 0, 1.0)
+    X = U.to_dev(indptr, indices, data, 20)
+    with pytest.raises(B.RscError):
+        B.rsc_normalize_total(X, float("nan"))
+    with pytest.raises(B.RscError):
+        B.rsc_gene_moments(X, transform=2)
+    with pytest.raises(B.RscError):
+        B.rsc_hvg_select(torch.zeros(4, dtype=torch.float64).cuda(), torch.zeros(4, dtype=torch.float64).cuda(), 0)
+    # too-small workspace is refused
+    import ctypes as C
+    L = B.lib()
+    cs = X.c_struct()
+    m = torch.empty(20, dtype=torch.float64, device="cuda")
+    rc = L.rsc_gene_moments(C.byref(cs), 0, 1, B._ptr(m), B._ptr(m), None, None, B._ptr(m), 8, None)
+    assert rc == B.RSC_ERR_WORKSPACE
