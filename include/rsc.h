@@ -58,12 +58,33 @@ typedef struct {
   float* data;           /* [nnz]; rewritten in place by normalize / log1p / fused    */
 } rsc_csr;
 
+/* Row split table (used by the streaming kernels to cut the gene axis into groups whose
+ * accumulators fit one SM's shared memory).  Columns are cut into K = ceil(n_cols /
+ * RSC_SPLIT_WIDTH) blocks; the table holds, for every row, K + 1 uint32 values
+ *     splits[row * (K + 1) + k] = #{stored entries of the row with column < k * RSC_SPLIT_WIDTH}
+ * (so splits[row][0] = 0 and splits[row][K] = the row length).  It is only meaningful for
+ * rows with ascending column indices (RSC_CSR_SORTED).  rsc_qc_metrics can emit it for free
+ * while it streams the matrix; rsc_row_splits computes it on its own (binary searches). */
+#define RSC_SPLIT_SHIFT 10
+#define RSC_SPLIT_WIDTH (1 << RSC_SPLIT_SHIFT)
+/* number of uint32 elements of the table */
+size_t rsc_row_splits_count(int64_t n_rows, int32_t n_cols);
+int rsc_row_splits(const rsc_csr* X, uint32_t* row_splits, void* stream);
+
 const char* rsc_last_error(void);
 /* Library version, "major.minor.patch". */
 const char* rsc_version(void);
 /* Number of CUDA kernels this library has launched so far in the calling process (host-side
  * counter; memsets / memcpys are not counted).  Used by bench.py to report gpu_launches. */
 uint64_t rsc_kernel_launch_count(void);
+/* Process-wide tuning / testing knobs (not needed in normal use; defaults in brackets):
+ *   "fused_row_budget" [4000]  rows a CTA of the fused pass takes between two flushes of its
+ *                              fixed-point accumulators (1..4092; 4096 rows cannot overflow)
+ *   "qc_row_budget"    [65528] the same for the QC pass's 16-bit count fields (1..65528)
+ *   "grid_ctas"        [0]     CTAs of the streaming kernels, 0 = one per SM
+ *   "force_generic"    [0]     1 = always take the generic L2-atomic kernels
+ * Returns RSC_ERR_INVALID_ARG for an unknown key or a value out of range. */
+int rsc_set_option(const char* key, long long value);
 
 /* ---------------------------------------------------------------------------------
  * rsc_qc_metrics — per-cell and per-gene QC reductions.
@@ -78,13 +99,15 @@ uint64_t rsc_kernel_launch_count(void);
  *   gene_total_i64[j]      sum over column j of (int64) x
  * Values are truncated to integers before summation; counts must be < 2^24.
  * gene_flags: uint8[n_cols] or NULL (then M_i = 0, pct = 0 or NaN).
+ * row_splits: optional uint32[rsc_row_splits_count(n_rows, n_cols)] receiving the row split
+ *   table (see above); written only when X->flags has RSC_CSR_SORTED, else left untouched.
  * Outputs are fully overwritten (no accumulation into previous contents).
  * ------------------------------------------------------------------------------- */
 size_t rsc_qc_metrics_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
 int rsc_qc_metrics(const rsc_csr* X, const uint8_t* gene_flags,
                    int64_t* cell_total_i64, float* cell_total_f32, int32_t* cell_n_genes,
                    int64_t* cell_flag_total_i64, float* cell_flag_pct,
-                   int32_t* gene_n_cells, int64_t* gene_total_i64,
+                   int32_t* gene_n_cells, int64_t* gene_total_i64, uint32_t* row_splits,
                    void* ws, size_t ws_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------------
@@ -127,7 +150,13 @@ int rsc_gene_moments(const rsc_csr* X, int transform, int ddof,
  * sums of the ROUNDED float32 x'' (log scale) and/or x' (linear scale) are
  * accumulated in double precision.
  *   which_moments: bit0 RSC_MOMENTS_LOG -> mean_log/var_log, bit1 RSC_MOMENTS_LIN ->
- *   mean_lin/var_lin (the matching pointers are then required).
+ *   mean_lin/var_lin (the matching pointers are then required).  By default the sums are
+ *   accumulated on chip in 64-bit fixed point (order-independent; every addend keeps >= 31
+ *   significant bits for non-negative data with x' >= target_sum * 2^-30, see DESIGN.md
+ *   section 5); bit2 RSC_MOMENTS_FP64_ACC selects double-precision accumulators instead
+ *   (any value range, slower).  Data must be non-negative for the fixed-point path.
+ *   row_splits: optional row split table of X (from rsc_qc_metrics / rsc_row_splits);
+ *   NULL -> computed into the workspace when needed.
  *   cell_total_i64 is required (from rsc_qc_metrics).
  *   gene_n_cells: optional hint (from rsc_qc_metrics) used to balance the gene
  *   ranges of the shared-memory accumulators; results do not depend on it.
@@ -137,9 +166,11 @@ int rsc_gene_moments(const rsc_csr* X, int transform, int ddof,
  * ------------------------------------------------------------------------------- */
 #define RSC_MOMENTS_LOG 1
 #define RSC_MOMENTS_LIN 2
+#define RSC_MOMENTS_FP64_ACC 4
 size_t rsc_normalize_log1p_moments_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
 int rsc_normalize_log1p_moments(rsc_csr* X, float target_sum, const int64_t* cell_total_i64,
-                                const int32_t* gene_n_cells, int which_moments, int ddof,
+                                const int32_t* gene_n_cells, const uint32_t* row_splits,
+                                int which_moments, int ddof,
                                 double* mean_log, double* var_log,
                                 double* mean_lin, double* var_lin, double* gene_sums_out,
                                 void* ws, size_t ws_bytes, void* stream);

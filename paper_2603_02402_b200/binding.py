@@ -25,10 +25,13 @@ RSC_ERR_UNSUPPORTED = -4
 RSC_CSR_SORTED = 1
 RSC_MOMENTS_LOG = 1
 RSC_MOMENTS_LIN = 2
+RSC_MOMENTS_FP64_ACC = 4
+RSC_SPLIT_WIDTH = 1024
 RSC_HVG_SEURAT_LOG = 1
 
 EXPORTS = [
     "rsc_last_error", "rsc_version", "rsc_kernel_launch_count",
+    "rsc_row_splits_count", "rsc_row_splits", "rsc_set_option",
     "rsc_qc_metrics_workspace_bytes", "rsc_qc_metrics",
     "rsc_normalize_total", "rsc_log1p",
     "rsc_gene_moments_workspace_bytes", "rsc_gene_moments",
@@ -86,7 +89,7 @@ def lib() -> C.CDLL:
     L.rsc_kernel_launch_count.restype = C.c_uint64
     for name in EXPORTS:
         f = getattr(L, name)
-        if name.endswith("_workspace_bytes"):
+        if name.endswith("_workspace_bytes") or name == "rsc_row_splits_count":
             f.restype = C.c_size_t
         elif name not in ("rsc_last_error", "rsc_version", "rsc_kernel_launch_count"):
             f.restype = C.c_int
@@ -97,11 +100,14 @@ def lib() -> C.CDLL:
     L.rsc_hvg_select_workspace_bytes.argtypes = [i32, i32]
     L.rsc_preprocess_workspace_bytes.argtypes = [i64, i32, i64, i32]
     L.rsc_preprocess_host_workspace_bytes.argtypes = [i64, i32, i64, i32]
-    L.rsc_qc_metrics.argtypes = [p] + [p] * 8 + [p, sz, p]
+    L.rsc_set_option.argtypes = [C.c_char_p, C.c_longlong]
+    L.rsc_row_splits_count.argtypes = [i64, i32]
+    L.rsc_row_splits.argtypes = [p, p, p]
+    L.rsc_qc_metrics.argtypes = [p] + [p] * 9 + [p, sz, p]
     L.rsc_normalize_total.argtypes = [p, flt, p, p, p]
     L.rsc_log1p.argtypes = [p, p]
     L.rsc_gene_moments.argtypes = [p, C.c_int, C.c_int, p, p, p, p, p, sz, p]
-    L.rsc_normalize_log1p_moments.argtypes = [p, flt, p, p, C.c_int, C.c_int, p, p, p, p, p, p, sz, p]
+    L.rsc_normalize_log1p_moments.argtypes = [p, flt, p, p, p, C.c_int, C.c_int, p, p, p, p, p, p, sz, p]
     L.rsc_moments_finalize.argtypes = [i32, i64, C.c_int, p, p, p, p, p]
     L.rsc_hvg_select.argtypes = [i32, p, p, i32, i32, C.c_int, p, p, p, p, p, p, p, p, sz, p]
     L.rsc_preprocess.argtypes = [p, p, p, p, p, sz, p]
@@ -174,7 +180,26 @@ def rsc_kernel_launch_count() -> int:
     return int(lib().rsc_kernel_launch_count())
 
 
-def rsc_qc_metrics(X: Csr, gene_flags: Optional[torch.Tensor] = None, stream=None) -> dict:
+def rsc_set_option(key: str, value: int) -> None:
+    _check(lib().rsc_set_option(key.encode(), int(value)))
+
+
+def rsc_row_splits_count(n_rows: int, n_cols: int) -> int:
+    return int(lib().rsc_row_splits_count(int(n_rows), int(n_cols)))
+
+
+def rsc_row_splits(X: Csr, stream=None) -> torch.Tensor:
+    """Row split table of a sorted CSR matrix (uint32 values in an int32 tensor)."""
+    _need_cuda(X)
+    out = torch.empty(max(1, rsc_row_splits_count(X.n_rows, X.n_cols)), dtype=torch.int32,
+                      device=X.device)
+    cs = X.c_struct()
+    _check(lib().rsc_row_splits(C.byref(cs), _ptr(out), _stream(stream)))
+    return out
+
+
+def rsc_qc_metrics(X: Csr, gene_flags: Optional[torch.Tensor] = None, stream=None,
+                   with_row_splits: bool = False) -> dict:
     _need_cuda(X)
     L, dev, n, G = lib(), X.device, X.n_rows, X.n_cols
     out = dict(
@@ -189,9 +214,14 @@ def rsc_qc_metrics(X: Csr, gene_flags: Optional[torch.Tensor] = None, stream=Non
     nb = L.rsc_qc_metrics_workspace_bytes(n, G, X.nnz)
     ws = _ws(nb, dev)
     cs = X.c_struct()
+    splits = None
+    if with_row_splits and X.sorted_indices:
+        splits = torch.empty(max(1, rsc_row_splits_count(n, G)), dtype=torch.int32, device=dev)
     _check(L.rsc_qc_metrics(C.byref(cs), _ptr(gene_flags), *[_ptr(out[k]) for k in (
         "cell_total_i64", "cell_total_f32", "cell_n_genes", "cell_flag_total_i64", "cell_flag_pct",
-        "gene_n_cells", "gene_total_i64")], _ptr(ws), ws.numel(), _stream(stream)))
+        "gene_n_cells", "gene_total_i64")], _ptr(splits), _ptr(ws), ws.numel(), _stream(stream)))
+    if splits is not None:
+        out["row_splits"] = splits
     return out
 
 
@@ -226,7 +256,8 @@ def rsc_gene_moments(X: Csr, transform: int = 0, ddof: int = 1, stream=None) -> 
 def rsc_normalize_log1p_moments(X: Csr, target_sum: float, cell_total_i64: torch.Tensor,
                                 gene_n_cells: Optional[torch.Tensor] = None,
                                 which_moments: int = RSC_MOMENTS_LOG | RSC_MOMENTS_LIN,
-                                ddof: int = 1, return_sums: bool = False, stream=None) -> dict:
+                                ddof: int = 1, return_sums: bool = False, stream=None,
+                                row_splits: Optional[torch.Tensor] = None) -> dict:
     _need_cuda(X)
     L, dev, G = lib(), X.device, X.n_cols
     out = {}
@@ -241,8 +272,8 @@ def rsc_normalize_log1p_moments(X: Csr, target_sum: float, cell_total_i64: torch
     ws = _ws(L.rsc_normalize_log1p_moments_workspace_bytes(X.n_rows, G, X.nnz), dev)
     cs = X.c_struct()
     _check(L.rsc_normalize_log1p_moments(
-        C.byref(cs), float(target_sum), _ptr(cell_total_i64), _ptr(gene_n_cells), which_moments,
-        ddof, _ptr(out.get("mean_log")), _ptr(out.get("var_log")), _ptr(out.get("mean_lin")),
+        C.byref(cs), float(target_sum), _ptr(cell_total_i64), _ptr(gene_n_cells), _ptr(row_splits),
+        which_moments, ddof, _ptr(out.get("mean_log")), _ptr(out.get("var_log")), _ptr(out.get("mean_lin")),
         _ptr(out.get("var_lin")), _ptr(out.get("sums")), _ptr(ws), ws.numel(), _stream(stream)))
     return out
 
@@ -338,34 +369,36 @@ class Preprocessor:
         _need_cuda(X)
         L, o, p = lib(), self.out, self.params
         st = torch.cuda.current_stream() if stream is None else stream
-        sp = C.c_void_p(st.cuda_stream)
+        sp_ = C.c_void_p(st.cuda_stream)
         cs = X.c_struct()
         if not hasattr(self, "_stage_ws"):
             n, G, nnz = X.n_rows, X.n_cols, X.nnz
             self._stage_ws = [_ws(L.rsc_qc_metrics_workspace_bytes(n, G, nnz), X.device),
                               _ws(L.rsc_normalize_log1p_moments_workspace_bytes(n, G, nnz), X.device),
-                              _ws(L.rsc_hvg_select_workspace_bytes(G, p.n_bins), X.device)]
-        w0, w1, w2 = self._stage_ws
+                              _ws(L.rsc_hvg_select_workspace_bytes(G, p.n_bins), X.device),
+                              torch.empty(max(1, rsc_row_splits_count(n, G)), dtype=torch.int32,
+                                          device=X.device) if X.sorted_indices else None]
+        w0, w1, w2, sp = self._stage_ws
         if events:
             events[0].record(st)
         _check(L.rsc_qc_metrics(C.byref(cs), _ptr(gene_flags), _ptr(o["cell_total_i64"]),
                                 _ptr(o["cell_total_f32"]), _ptr(o["cell_n_genes"]),
                                 _ptr(o["cell_flag_total_i64"]), _ptr(o["cell_flag_pct"]),
-                                _ptr(o["gene_n_cells"]), _ptr(o["gene_total_i64"]), _ptr(w0),
-                                w0.numel(), sp))
+                                _ptr(o["gene_n_cells"]), _ptr(o["gene_total_i64"]), _ptr(sp),
+                                _ptr(w0), w0.numel(), sp_))
         if events:
             events[1].record(st)
         _check(L.rsc_normalize_log1p_moments(
-            C.byref(cs), p.target_sum, _ptr(o["cell_total_i64"]), _ptr(o["gene_n_cells"]),
+            C.byref(cs), p.target_sum, _ptr(o["cell_total_i64"]), _ptr(o["gene_n_cells"]), _ptr(sp),
             p.which_moments, p.ddof, _ptr(o["mean_log"]), _ptr(o["var_log"]), _ptr(o["mean_lin"]),
-            _ptr(o["var_lin"]), None, _ptr(w1), w1.numel(), sp))
+            _ptr(o["var_lin"]), None, _ptr(w1), w1.numel(), sp_))
         if events:
             events[2].record(st)
         hm, hv = (o["mean_lin"], o["var_lin"]) if p.hvg_on_linear else (o["mean_log"], o["var_log"])
         _check(L.rsc_hvg_select(X.n_cols, _ptr(hm), _ptr(hv), p.n_top, p.n_bins, p.hvg_flags,
                                 _ptr(o["hvg_mean_t"]), _ptr(o["hvg_disp"]), _ptr(o["hvg_disp_norm"]),
                                 _ptr(o["hvg_bin"]), _ptr(o["hvg_mask"]), _ptr(o["hvg_indices"]),
-                                _ptr(o["hvg_count"]), _ptr(w2), w2.numel(), sp))
+                                _ptr(o["hvg_count"]), _ptr(w2), w2.numel(), sp_))
         if events:
             events[3].record(st)
         return self.out

@@ -11,6 +11,7 @@ namespace rsc {
 
 static thread_local char g_err[512] = "";
 unsigned long long g_launch_count = 0;
+Options g_opt;
 
 void set_error(const char* fmt, ...) {
   va_list ap;
@@ -63,28 +64,12 @@ static int check_ws(const char* who, void* ws, size_t have, size_t need) {
 }
 
 // implemented in generic.cu
-int launch_qc_generic(const rsc_csr&, const uint8_t*, int64_t*, float*, int32_t*, int64_t*, float*,
-                      int32_t*, int64_t*, cudaStream_t);
 int launch_moments_generic(const rsc_csr&, int, double*, double*, cudaStream_t);
-int launch_fused_generic(const rsc_csr&, float, const int64_t*, int, double*, double*, double*,
-                         double*, cudaStream_t);
 int finalize_moments(int32_t, int64_t, int, const double*, const double*, double*, double*,
                      cudaStream_t);
 
-size_t qc_workspace_bytes(int64_t, int32_t, int64_t) { return 256; }
 size_t moments_workspace_bytes(int64_t, int32_t n_cols, int64_t) {
   return 2 * align_up(sizeof(double) * (size_t)n_cols, 256);
-}
-size_t fused_workspace_bytes(int64_t, int32_t n_cols, int64_t) {
-  return 4 * align_up(sizeof(double) * (size_t)n_cols, 256);
-}
-
-int launch_qc(const rsc_csr& X, const uint8_t* gene_flags, int64_t* cell_total_i64,
-              float* cell_total_f32, int32_t* cell_n_genes, int64_t* cell_flag_total_i64,
-              float* cell_flag_pct, int32_t* gene_n_cells, int64_t* gene_total_i64, void*, size_t,
-              cudaStream_t st) {
-  return launch_qc_generic(X, gene_flags, cell_total_i64, cell_total_f32, cell_n_genes,
-                           cell_flag_total_i64, cell_flag_pct, gene_n_cells, gene_total_i64, st);
 }
 
 int launch_moments(const rsc_csr& X, int transform, int ddof, double* mean, double* var,
@@ -98,30 +83,6 @@ int launch_moments(const rsc_csr& X, int transform, int ddof, double* mean, doub
   return finalize_moments(X.n_cols, X.n_rows, ddof, S1, S2, mean, var, st);
 }
 
-int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i64,
-                 const int32_t* /*gene_n_cells*/, int which, int ddof, double* mean_log,
-                 double* var_log, double* mean_lin, double* var_lin, double* sums_out, void* ws,
-                 size_t, cudaStream_t st) {
-  const size_t gsz = align_up(sizeof(double) * (size_t)X.n_cols, 256);
-  unsigned char* w = static_cast<unsigned char*>(ws);
-  const size_t G = (size_t)X.n_cols;
-  double* S1log = sums_out ? sums_out : reinterpret_cast<double*>(w);
-  double* S2log = sums_out ? sums_out + G : reinterpret_cast<double*>(w + gsz);
-  double* S1lin = sums_out ? sums_out + 2 * G : reinterpret_cast<double*>(w + 2 * gsz);
-  double* S2lin = sums_out ? sums_out + 3 * G : reinterpret_cast<double*>(w + 3 * gsz);
-  int rc = launch_fused_generic(X, target_sum, cell_total_i64, which, S1log, S2log, S1lin, S2lin, st);
-  if (rc != RSC_OK) return rc;
-  if (which & RSC_MOMENTS_LOG) {
-    rc = finalize_moments(X.n_cols, X.n_rows, ddof, S1log, S2log, mean_log, var_log, st);
-    if (rc != RSC_OK) return rc;
-  }
-  if (which & RSC_MOMENTS_LIN) {
-    rc = finalize_moments(X.n_cols, X.n_rows, ddof, S1lin, S2lin, mean_lin, var_lin, st);
-    if (rc != RSC_OK) return rc;
-  }
-  return RSC_OK;
-}
-
 }  // namespace rsc
 
 using namespace rsc;
@@ -132,22 +93,56 @@ const char* rsc_last_error(void) { return g_err; }
 const char* rsc_version(void) { return "0.1.0"; }
 uint64_t rsc_kernel_launch_count(void) { return g_launch_count; }
 
+int rsc_set_option(const char* key, long long value) {
+  RSC_CHECK_ARG(key != nullptr, "rsc_set_option: key is NULL");
+  if (!strcmp(key, "fused_row_budget")) {
+    RSC_CHECK_ARG(value >= 1 && value <= 4092, "rsc_set_option: fused_row_budget must be in [1, 4092]");
+    g_opt.fused_row_budget = (int)value;
+  } else if (!strcmp(key, "qc_row_budget")) {
+    RSC_CHECK_ARG(value >= 1 && value <= 65528, "rsc_set_option: qc_row_budget must be in [1, 65528]");
+    g_opt.qc_row_budget = (int)value;
+  } else if (!strcmp(key, "grid_ctas")) {
+    RSC_CHECK_ARG(value >= 0 && value <= 65535, "rsc_set_option: grid_ctas must be in [0, 65535]");
+    g_opt.grid_ctas = (int)value;
+  } else if (!strcmp(key, "force_generic")) {
+    g_opt.force_generic = value != 0;
+  } else {
+    set_error("rsc_set_option: unknown key '%s'", key);
+    return RSC_ERR_INVALID_ARG;
+  }
+  return RSC_OK;
+}
+
 size_t rsc_qc_metrics_workspace_bytes(int64_t n, int32_t G, int64_t nnz) {
   return qc_workspace_bytes(n, G, nnz);
 }
 
+size_t rsc_row_splits_count(int64_t n_rows, int32_t n_cols) {
+  if (n_rows < 0 || n_cols <= 0) return 0;
+  return (size_t)n_rows * ((size_t)split_blocks(n_cols) + 1);
+}
+
+int rsc_row_splits(const rsc_csr* X, uint32_t* row_splits, void* stream) {
+  int rc = check_csr(X, "rsc_row_splits", false);
+  if (rc) return rc;
+  RSC_CHECK_ARG(row_splits != nullptr, "rsc_row_splits: row_splits is NULL");
+  if ((rc = check_device())) return rc;
+  return launch_row_splits(*X, row_splits, static_cast<cudaStream_t>(stream));
+}
+
 int rsc_qc_metrics(const rsc_csr* X, const uint8_t* gene_flags, int64_t* cell_total_i64,
                    float* cell_total_f32, int32_t* cell_n_genes, int64_t* cell_flag_total_i64,
-                   float* cell_flag_pct, int32_t* gene_n_cells, int64_t* gene_total_i64, void* ws,
-                   size_t ws_bytes, void* stream) {
+                   float* cell_flag_pct, int32_t* gene_n_cells, int64_t* gene_total_i64,
+                   uint32_t* row_splits, void* ws, size_t ws_bytes, void* stream) {
   int rc = check_csr(X, "rsc_qc_metrics", true);
   if (rc) return rc;
   if ((rc = check_device())) return rc;
   if ((rc = check_ws("rsc_qc_metrics", ws, ws_bytes, qc_workspace_bytes(X->n_rows, X->n_cols, X->nnz))))
     return rc;
+  if (!(X->flags & RSC_CSR_SORTED)) row_splits = nullptr;
   return launch_qc(*X, gene_flags, cell_total_i64, cell_total_f32, cell_n_genes,
-                   cell_flag_total_i64, cell_flag_pct, gene_n_cells, gene_total_i64, ws, ws_bytes,
-                   static_cast<cudaStream_t>(stream));
+                   cell_flag_total_i64, cell_flag_pct, gene_n_cells, gene_total_i64, row_splits, ws,
+                   ws_bytes, static_cast<cudaStream_t>(stream));
 }
 
 int rsc_normalize_total(rsc_csr* X, float target_sum, const int64_t* cell_total_i64,
@@ -195,8 +190,8 @@ size_t rsc_normalize_log1p_moments_workspace_bytes(int64_t n, int32_t G, int64_t
 }
 
 int rsc_normalize_log1p_moments(rsc_csr* X, float target_sum, const int64_t* cell_total_i64,
-                                const int32_t* gene_n_cells, int which_moments, int ddof,
-                                double* mean_log, double* var_log, double* mean_lin,
+                                const int32_t* gene_n_cells, const uint32_t* row_splits,
+                                int which_moments, int ddof, double* mean_log, double* var_log, double* mean_lin,
                                 double* var_lin, double* gene_sums_out, void* ws, size_t ws_bytes,
                                 void* stream) {
   int rc = check_csr(X, "rsc_normalize_log1p_moments", true);
@@ -204,9 +199,9 @@ int rsc_normalize_log1p_moments(rsc_csr* X, float target_sum, const int64_t* cel
   RSC_CHECK_ARG(isfinite(target_sum) && target_sum > 0.0f,
                 "rsc_normalize_log1p_moments: target_sum must be finite and > 0");
   RSC_CHECK_ARG(cell_total_i64 != nullptr, "rsc_normalize_log1p_moments: cell_total_i64 is required");
-  RSC_CHECK_ARG((which_moments & ~3) == 0, "rsc_normalize_log1p_moments: bad which_moments");
+  RSC_CHECK_ARG((which_moments & ~7) == 0, "rsc_normalize_log1p_moments: bad which_moments");
   RSC_CHECK_ARG(ddof == 0 || ddof == 1, "rsc_normalize_log1p_moments: ddof must be 0 or 1");
-  RSC_CHECK_ARG(which_moments == 0 || X->n_rows - ddof > 0,
+  RSC_CHECK_ARG((which_moments & 3) == 0 || X->n_rows - ddof > 0,
                 "rsc_normalize_log1p_moments: n_rows - ddof must be > 0");
   RSC_CHECK_ARG(!(which_moments & RSC_MOMENTS_LOG) || (mean_log && var_log),
                 "rsc_normalize_log1p_moments: mean_log / var_log required with RSC_MOMENTS_LOG");
@@ -216,8 +211,8 @@ int rsc_normalize_log1p_moments(rsc_csr* X, float target_sum, const int64_t* cel
   if ((rc = check_ws("rsc_normalize_log1p_moments", ws, ws_bytes,
                      fused_workspace_bytes(X->n_rows, X->n_cols, X->nnz))))
     return rc;
-  return launch_fused(*X, target_sum, cell_total_i64, gene_n_cells, which_moments, ddof, mean_log,
-                      var_log, mean_lin, var_lin, gene_sums_out, ws, ws_bytes,
+  return launch_fused(*X, target_sum, cell_total_i64, gene_n_cells, row_splits, which_moments, ddof,
+                      mean_log, var_log, mean_lin, var_lin, gene_sums_out, ws, ws_bytes,
                       static_cast<cudaStream_t>(stream));
 }
 

@@ -27,6 +27,7 @@ struct Carver {
 struct ChainWs {
   int64_t* cell_total;
   int32_t* gene_n_cells;
+  uint32_t* splits;
   double *mean_log, *var_log, *mean_lin, *var_lin;
   void *qc_ws, *fused_ws, *hvg_ws;
   size_t qc_bytes, fused_bytes, hvg_bytes;
@@ -38,6 +39,7 @@ static ChainWs carve_chain(void* ws, int64_t n, int32_t G, int64_t nnz, int32_t 
   ChainWs w;
   w.cell_total = c.take<int64_t>((size_t)n);
   w.gene_n_cells = c.take<int32_t>((size_t)G);
+  w.splits = c.take<uint32_t>(rsc_row_splits_count(n, G));
   w.mean_log = c.take<double>((size_t)G);
   w.var_log = c.take<double>((size_t)G);
   w.mean_lin = c.take<double>((size_t)G);
@@ -58,7 +60,8 @@ static int check_params(const rsc_params* p, const char* who) {
   RSC_CHECK_ARG(p->n_top >= 1, "%s: n_top < 1", who);
   RSC_CHECK_ARG(p->n_bins >= 1 && p->n_bins <= 4096, "%s: n_bins must be in [1, 4096]", who);
   RSC_CHECK_ARG(p->ddof == 0 || p->ddof == 1, "%s: ddof must be 0 or 1", who);
-  RSC_CHECK_ARG(p->which_moments >= 1 && p->which_moments <= 3, "%s: which_moments must be 1..3", who);
+  RSC_CHECK_ARG((p->which_moments & 3) != 0 && (p->which_moments & ~7) == 0,
+                "%s: which_moments must request RSC_MOMENTS_LOG and / or RSC_MOMENTS_LIN", who);
   RSC_CHECK_ARG(p->hvg_on_linear ? (p->which_moments & RSC_MOMENTS_LIN)
                                  : (p->which_moments & RSC_MOMENTS_LOG),
                 "%s: which_moments does not produce the moments HVG is asked to consume", who);
@@ -75,11 +78,12 @@ static int run_chain(rsc_csr* X, const uint8_t* gene_flags, const rsc_params* pr
   double* mean_lin = out->mean_lin ? out->mean_lin : w.mean_lin;
   double* var_lin = out->var_lin ? out->var_lin : w.var_lin;
 
+  uint32_t* splits = (X->flags & RSC_CSR_SORTED) ? w.splits : nullptr;
   int rc = launch_qc(*X, gene_flags, cell_total, out->cell_total_f32, out->cell_n_genes,
                      out->cell_flag_total_i64, out->cell_flag_pct, gene_n_cells,
-                     out->gene_total_i64, w.qc_ws, w.qc_bytes, st);
+                     out->gene_total_i64, splits, w.qc_ws, w.qc_bytes, st);
   if (rc) return rc;
-  rc = launch_fused(*X, prm->target_sum, cell_total, gene_n_cells, prm->which_moments, prm->ddof,
+  rc = launch_fused(*X, prm->target_sum, cell_total, gene_n_cells, splits, prm->which_moments, prm->ddof,
                     mean_log, var_log, mean_lin, var_lin, nullptr, w.fused_ws, w.fused_bytes, st);
   if (rc) return rc;
   const double* hm = prm->hvg_on_linear ? mean_lin : mean_log;

@@ -12,6 +12,10 @@ namespace rsc {
 
 constexpr int kNumSMs = 148;       // B200: 2 dies x 74 SMs (grid sizing)
 constexpr int kWarp = 32;
+constexpr size_t kMaxDynSmem = 231424;   // 226 KB dynamic (+ static < 1 KB) <= 227 KB opt-in limit per CTA
+
+// number of column blocks K of the row split table (RSC_SPLIT_WIDTH columns each)
+inline int split_blocks(int32_t n_cols) { return (n_cols + RSC_SPLIT_WIDTH - 1) >> RSC_SPLIT_SHIFT; }
 
 void set_error(const char* fmt, ...);
 
@@ -32,6 +36,15 @@ void set_error(const char* fmt, ...);
       return RSC_ERR_CUDA;                                                          \
     }                                                                               \
   } while (0)
+
+// run-time tunables (rsc_set_option): defaults are the shipped configuration
+struct Options {
+  int fused_row_budget = 4000;    // rows a fused-pass CTA takes between flushes (<= 4092)
+  int qc_row_budget = 65528;      // rows a QC CTA takes between flushes (< 65536 - 4)
+  int grid_ctas = 0;              // CTAs of the streaming kernels; 0 = one per SM
+  int force_generic = 0;          // 1: always use the generic L2-atomic kernels
+};
+extern Options g_opt;
 
 extern unsigned long long g_launch_count;   // kernels launched by this library (host counter)
 
@@ -55,9 +68,10 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 // ---- launchers implemented in the kernel translation units -------------------------
 int launch_qc(const rsc_csr& X, const uint8_t* gene_flags, int64_t* cell_total_i64,
               float* cell_total_f32, int32_t* cell_n_genes, int64_t* cell_flag_total_i64,
-              float* cell_flag_pct, int32_t* gene_n_cells, int64_t* gene_total_i64, void* ws,
-              size_t ws_bytes, cudaStream_t st);
+              float* cell_flag_pct, int32_t* gene_n_cells, int64_t* gene_total_i64,
+              uint32_t* row_splits, void* ws, size_t ws_bytes, cudaStream_t st);
 size_t qc_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
+int launch_row_splits(const rsc_csr& X, uint32_t* splits, cudaStream_t st);
 
 int launch_normalize(const rsc_csr& X, float target_sum, const int64_t* cell_total_i64,
                      float* cell_scale_out, cudaStream_t st);
@@ -69,7 +83,8 @@ int launch_moments(const rsc_csr& X, int transform, int ddof, double* mean, doub
 size_t moments_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
 
 int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i64,
-                 const int32_t* gene_n_cells, int which, int ddof, double* mean_log,
+                 const int32_t* gene_n_cells, const uint32_t* row_splits, int which, int ddof,
+                 double* mean_log,
                  double* var_log, double* mean_lin, double* var_lin, double* sums_out, void* ws,
                  size_t ws_bytes, cudaStream_t st);
 int finalize_moments(int32_t G, int64_t n, int ddof, const double* S1, const double* S2,
@@ -91,6 +106,27 @@ __device__ __forceinline__ T warp_sum(T v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return v;
+}
+
+// x'' = log(1 + x') in float32, shared by rsc_log1p and the fused pass so that
+// both write bit-identical values.  x >= 0.25: MUFU lg2 of the rounded 1 + x (absolute error
+// <= 2^-22 * ln 2 + 2^-24, i.e. <= 1e-6 relative there, ~1 ulp for typical x'' of 1..3);
+// |x| < 0.25: x * (1 - x/2 + x^2/3 - ... - x^9/10), truncation < 1e-7 relative.
+// The stated tolerance on x'' is 1e-5 relative (north_star).
+__device__ __forceinline__ float log1p_f32(float x) {
+  if (x >= 0.25f) return __logf(1.0f + x);
+  if (x < -0.25f) return log1pf(x);
+  float p = -0.1f;
+  p = fmaf(p, x, 1.0f / 9.0f);
+  p = fmaf(p, x, -0.125f);
+  p = fmaf(p, x, 1.0f / 7.0f);
+  p = fmaf(p, x, -1.0f / 6.0f);
+  p = fmaf(p, x, 0.2f);
+  p = fmaf(p, x, -0.25f);
+  p = fmaf(p, x, 1.0f / 3.0f);
+  p = fmaf(p, x, -0.5f);
+  p = fmaf(p, x, 1.0f);
+  return x * p;
 }
 
 // scale_i of normalize_total: one float32 division, shared by the unfused and the fused

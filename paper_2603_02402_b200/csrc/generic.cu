@@ -119,12 +119,12 @@ log1p_kernel(float* __restrict__ data, int64_t nnz) {
   const int64_t nth = (int64_t)gridDim.x * blockDim.x;
   for (int64_t i = tid; i < nvec; i += nth) {
     float4 x = v[i];
-    x.x = log1pf(x.x); x.y = log1pf(x.y); x.z = log1pf(x.z); x.w = log1pf(x.w);
+    x.x = log1p_f32(x.x); x.y = log1p_f32(x.y); x.z = log1p_f32(x.z); x.w = log1p_f32(x.w);
     v[i] = x;
   }
   const int64_t tail0 = head + (nvec << 2);
-  if (tid < head) data[tid] = log1pf(data[tid]);
-  if (tid < nnz - tail0) data[tail0 + tid] = log1pf(data[tail0 + tid]);
+  if (tid < head) data[tid] = log1p_f32(data[tid]);
+  if (tid < nnz - tail0) data[tail0 + tid] = log1p_f32(data[tail0 + tid]);
 }
 
 int launch_log1p(const rsc_csr& X, cudaStream_t st) {
@@ -204,7 +204,7 @@ fused_generic_kernel(int64_t n_rows, const int64_t* __restrict__ indptr,
     const float scale = cell_scale(target_sum, cell_total[row]);
     for (int64_t p = beg + lane; p < end; p += 32) {
       const float xn = __fmul_rn(data[p], scale);
-      const float xl = log1pf(xn);
+      const float xl = log1p_f32(xn);
       const int j = indices[p];
       data[p] = xl;
       if (LOG) {

@@ -66,6 +66,8 @@ def preprocess_sharded(pp: "B.Preprocessor", X: "B.Csr", gene_flags: Optional[to
             w0=B._ws(L.rsc_qc_metrics_workspace_bytes(n, G, nnz), X.device),
             w1=B._ws(L.rsc_normalize_log1p_moments_workspace_bytes(n, G, nnz), X.device),
             w2=B._ws(L.rsc_hvg_select_workspace_bytes(G, p.n_bins), X.device),
+            splits=(torch.empty(max(1, B.rsc_row_splits_count(n, G)), dtype=torch.int32,
+                                device=X.device) if X.sorted_indices else None),
             sums=torch.zeros(4, G, dtype=torch.float64, device=X.device),
             n_total=global_cell_count(n, X.device, group))
     sh = pp._sh
@@ -75,13 +77,13 @@ def preprocess_sharded(pp: "B.Preprocessor", X: "B.Csr", gene_flags: Optional[to
                               B._ptr(o["cell_total_f32"]), B._ptr(o["cell_n_genes"]),
                               B._ptr(o["cell_flag_total_i64"]), B._ptr(o["cell_flag_pct"]),
                               B._ptr(o["gene_n_cells"]), B._ptr(o["gene_total_i64"]),
-                              B._ptr(sh["w0"]), sh["w0"].numel(), sp))
+                              B._ptr(sh["splits"]), B._ptr(sh["w0"]), sh["w0"].numel(), sp))
     allreduce_gene_stats({"n_cells": o["gene_n_cells"], "total": o["gene_total_i64"]}, {}, group)
     if events:
         events[1].record(st)
     B._check(L.rsc_normalize_log1p_moments(
         C.byref(cs), p.target_sum, B._ptr(o["cell_total_i64"]), B._ptr(o["gene_n_cells"]),
-        p.which_moments, p.ddof, B._ptr(o["mean_log"]), B._ptr(o["var_log"]),
+        B._ptr(sh["splits"]), p.which_moments, p.ddof, B._ptr(o["mean_log"]), B._ptr(o["var_log"]),
         B._ptr(o["mean_lin"]), B._ptr(o["var_lin"]), B._ptr(sh["sums"]), B._ptr(sh["w1"]),
         sh["w1"].numel(), sp))
     allreduce_gene_stats({}, {"sums": sh["sums"]}, group)

@@ -236,3 +236,129 @@ def test_errors_are_loud():
     m = torch.empty(20, dtype=torch.float64, device="cuda")
     rc = L.rsc_gene_moments(C.byref(cs), 0, 1, B._ptr(m), B._ptr(m), None, None, B._ptr(m), 8, None)
     assert rc == B.RSC_ERR_WORKSPACE
+
+
+# ----------------------------------------------------------------------------------------
+# streaming kernels: row split table, flush paths, accumulator modes
+# ----------------------------------------------------------------------------------------
+def _splits_ref(indptr, indices, G, width=1024):
+    """splits[row, k] = #{entries of the row with column < k * width} (definition in rsc.h)."""
+    K = (G + width - 1) // width
+    n = len(indptr) - 1
+    out = np.zeros((n, K + 1), dtype=np.int64)
+    for i in range(n):
+        cols = indices[indptr[i]:indptr[i + 1]]
+        for k in range(K + 1):
+            out[i, k] = int(np.sum(cols < k * width))
+    return out
+
+
+@pytest.mark.parametrize("n,G,seed,depth,er,eg", SMALL)
+def test_row_splits_qc_and_standalone(n, G, seed, depth, er, eg):
+    from paper_2603_02402_b200 import binding as B
+    indptr, indices, data, _ = synth.small_nb_csr(n, G, seed, depth, empty_rows=er, empty_genes=eg)
+    want = _splits_ref(indptr, indices, G)
+    X = U.to_dev(indptr, indices, data, G)
+    assert B.rsc_row_splits_count(n, G) == want.size
+    a = U.np_(B.rsc_row_splits(X)).astype(np.int64)[: want.size].reshape(want.shape)
+    q = B.rsc_qc_metrics(X, None, with_row_splits=True)
+    b = U.np_(q["row_splits"]).astype(np.int64)[: want.size].reshape(want.shape)
+    assert np.array_equal(a, want), "rsc_row_splits"
+    assert np.array_equal(b, want), "row splits emitted by rsc_qc_metrics"
+
+
+@pytest.fixture
+def small_budgets():
+    """Force many flushes of the CTA-private tables and a small grid (rsc_set_option)."""
+    from paper_2603_02402_b200 import binding as B
+    B.rsc_set_option("fused_row_budget", 8)
+    B.rsc_set_option("qc_row_budget", 8)
+    B.rsc_set_option("grid_ctas", 9)
+    yield
+    B.rsc_set_option("fused_row_budget", 4000)
+    B.rsc_set_option("qc_row_budget", 65528)
+    B.rsc_set_option("grid_ctas", 0)
+
+
+@pytest.mark.parametrize("n,G,seed,depth,er,eg", SMALL[2:])
+@pytest.mark.parametrize("which", [1, 2, 3, 7])
+def test_streaming_kernels_flush_paths(small_budgets, n, G, seed, depth, er, eg, which):
+    from paper_2603_02402_b200 import binding as B
+    indptr, indices, data, _ = synth.small_nb_csr(n, G, seed, depth, empty_rows=er, empty_genes=eg)
+    flags = _flags(G, seed)
+    want = O.qc_metrics(indptr, indices, data, G, flags)
+    X = U.to_dev(indptr, indices, data, G)
+    Xn = U.clone(X)
+    q = B.rsc_qc_metrics(X, torch.as_tensor(flags).cuda(), with_row_splits=True)
+    for k in ("cell_total_i64", "cell_n_genes", "cell_flag_total_i64", "gene_n_cells", "gene_total_i64"):
+        U.assert_int_equal(q[k], want[k], k)
+    s = 1e4
+    out = B.rsc_normalize_log1p_moments(X, s, q["cell_total_i64"], q["gene_n_cells"], which, 1,
+                                        row_splits=q["row_splits"])
+    xl_o = O.log1p(O.normalize_total(indptr, data, s)[0])
+    U.assert_f32_close(X.data, xl_o, "x''")
+    if which & 1:
+        mo, vo, _, _ = O.gene_moments(indptr, indices, U.np_(X.data), G, 0, 1)
+        U.assert_moments_close(out["mean_log"], out["var_log"], mo, vo, "log moments")
+    if which & 2:
+        B.rsc_normalize_total(Xn, s, q["cell_total_i64"])
+        mo, vo, _, _ = O.gene_moments(indptr, indices, U.np_(Xn.data), G, 0, 1)
+        U.assert_moments_close(out["mean_lin"], out["var_lin"], mo, vo, "lin moments")
+
+
+def test_fused_equals_unfused_bitwise_and_is_order_independent():
+    """The fused pass writes the very x'' that rsc_normalize_total + rsc_log1p write, and its
+    on-chip fixed-point sums do not depend on the order of the atomic adds; only the few
+    per-CTA partial sums are added to the global doubles in scheduling order (last-bit noise)."""
+    from paper_2603_02402_b200 import binding as B
+    indptr, indices, data, _ = synth.small_nb_csr(1500, 4099, 3, 0.4)
+    X = U.to_dev(indptr, indices, data, 4099)
+    Xu = U.clone(X)
+    q = B.rsc_qc_metrics(X)
+    out1 = B.rsc_normalize_log1p_moments(X, 1e4, q["cell_total_i64"], q["gene_n_cells"], 3, 1, return_sums=True)
+    B.rsc_normalize_total(Xu, 1e4, q["cell_total_i64"])
+    B.rsc_log1p(Xu)
+    assert torch.equal(X.data, Xu.data)
+    X2 = U.to_dev(indptr, indices, data, 4099)
+    B.rsc_set_option("grid_ctas", 37)
+    try:
+        out2 = B.rsc_normalize_log1p_moments(X2, 1e4, q["cell_total_i64"], None, 3, 1, return_sums=True)
+    finally:
+        B.rsc_set_option("grid_ctas", 0)
+    # per-CTA partial sums are added to the global doubles in a different order / split, so
+    # the totals agree to the last bits but need not be identical across grids
+    np.testing.assert_allclose(U.np_(out1["sums"]), U.np_(out2["sums"]), rtol=1e-14)
+    X3 = U.to_dev(indptr, indices, data, 4099)
+    out3 = B.rsc_normalize_log1p_moments(X3, 1e4, q["cell_total_i64"], q["gene_n_cells"], 3, 1, return_sums=True)
+    np.testing.assert_allclose(U.np_(out1["sums"]), U.np_(out3["sums"]), rtol=1e-14)
+
+
+def test_fixed_point_extreme_ranges():
+    """Rows whose totals differ by 2^20 (x' from ~1e-2 to target_sum) and both target sums: the
+    fixed-point windows keep every addend's 31 significant bits."""
+    from paper_2603_02402_b200 import binding as B
+    rng = np.random.default_rng(7)
+    n, G = 64, 3000
+    dense = np.zeros((n, G), dtype=np.float64)
+    for i in range(n):
+        k = rng.integers(1, 40)
+        cols = rng.choice(G, size=k, replace=False)
+        dense[i, cols] = rng.integers(1, 4, size=k)
+    dense[0, :] = 0; dense[0, 5] = 7                      # one gene takes the whole cell: x' = s
+    dense[1, :2000] = 500.0                               # T = 1e6: x' = s / 2000 * ... tiny
+    dense[2, 5] = 1.0; dense[2, 100:1100] = 1000.0        # x' of gene 5 ~ s * 1e-6
+    indptr = np.zeros(n + 1, dtype=np.int64)
+    r, c = np.nonzero(dense)
+    np.cumsum(np.bincount(r, minlength=n), out=indptr[1:])
+    indices = c.astype(np.int32); data = dense[r, c].astype(np.float32)
+    for s in (1e4, 1e6):
+        for which in (3, 7):
+            X = U.to_dev(indptr, indices, data, G)
+            Xn = U.clone(X)
+            q = B.rsc_qc_metrics(X)
+            out = B.rsc_normalize_log1p_moments(X, s, q["cell_total_i64"], q["gene_n_cells"], which, 1)
+            mo, vo, _, _ = O.gene_moments(indptr, indices, U.np_(X.data), G, 0, 1)
+            U.assert_moments_close(out["mean_log"], out["var_log"], mo, vo, f"log s={s} which={which}")
+            B.rsc_normalize_total(Xn, s, q["cell_total_i64"])
+            mo, vo, _, _ = O.gene_moments(indptr, indices, U.np_(Xn.data), G, 0, 1)
+            U.assert_moments_close(out["mean_lin"], out["var_lin"], mo, vo, f"lin s={s} which={which}")
