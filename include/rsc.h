@@ -80,7 +80,7 @@ uint64_t rsc_kernel_launch_count(void);
 /* Process-wide tuning / testing knobs (not needed in normal use; defaults in brackets):
  *   "fused_row_budget" [4000]  rows a CTA of the fused pass takes between two flushes of its
  *                              fixed-point accumulators (1..4092; 4096 rows cannot overflow)
- *   "qc_row_budget"    [65528] the same for the QC pass's 16-bit count fields (1..65528)
+ *   "qc_row_budget"    [2043]  the same for the QC pass's 11-bit count fields (1..2043)
  *   "grid_ctas"        [0]     CTAs of the streaming kernels, 0 = one per SM
  *   "force_generic"    [0]     1 = always take the generic L2-atomic kernels
  * Returns RSC_ERR_INVALID_ARG for an unknown key or a value out of range. */

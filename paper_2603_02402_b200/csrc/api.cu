@@ -99,7 +99,7 @@ int rsc_set_option(const char* key, long long value) {
     RSC_CHECK_ARG(value >= 1 && value <= 4092, "rsc_set_option: fused_row_budget must be in [1, 4092]");
     g_opt.fused_row_budget = (int)value;
   } else if (!strcmp(key, "qc_row_budget")) {
-    RSC_CHECK_ARG(value >= 1 && value <= 65528, "rsc_set_option: qc_row_budget must be in [1, 65528]");
+    RSC_CHECK_ARG(value >= 1 && value <= 2043, "rsc_set_option: qc_row_budget must be in [1, 2043]");
     g_opt.qc_row_budget = (int)value;
   } else if (!strcmp(key, "grid_ctas")) {
     RSC_CHECK_ARG(value >= 0 && value <= 65535, "rsc_set_option: grid_ctas must be in [0, 65535]");

@@ -276,7 +276,7 @@ def small_budgets():
     B.rsc_set_option("grid_ctas", 9)
     yield
     B.rsc_set_option("fused_row_budget", 4000)
-    B.rsc_set_option("qc_row_budget", 65528)
+    B.rsc_set_option("qc_row_budget", 2043)
     B.rsc_set_option("grid_ctas", 0)
 
 
