@@ -113,8 +113,13 @@ __device__ __forceinline__ T warp_sum(T v) {
 // <= 2^-22 * ln 2 + 2^-24, i.e. <= 1e-6 relative there, ~1 ulp for typical x'' of 1..3);
 // |x| < 0.25: x * (1 - x/2 + x^2/3 - ... - x^9/10), truncation < 1e-7 relative.
 // The stated tolerance on x'' is 1e-5 relative (north_star).
+__device__ __forceinline__ float log1p_ge_quarter(float x) {      // x >= 0.25 (1 + x is normal)
+  float l;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l) : "f"(__fadd_rn(1.0f, x)));
+  return __fmul_rn(l, 0.693147182f);
+}
 __device__ __forceinline__ float log1p_f32(float x) {
-  if (x >= 0.25f) return __logf(1.0f + x);
+  if (x >= 0.25f) return log1p_ge_quarter(x);
   if (x < -0.25f) return log1pf(x);
   float p = -0.1f;
   p = fmaf(p, x, 1.0f / 9.0f);

@@ -5,44 +5,60 @@
 // itself is BASELINE.json north_star's, not the paper's.  12 B / nnz of DRAM traffic.
 //
 // Design:
-//   * Gene-range groups.  G genes x 4..5 64-bit accumulators do not fit one SM's shared
+//   * Gene-range groups.  G genes x 20..40 B of accumulators do not fit one SM's shared
 //     memory, so the columns are cut into groups of `fine_per_group` blocks of
 //     RSC_SPLIT_WIDTH genes; a CTA serves ONE group and keeps that group's accumulators
 //     (<= 227 KB) private.  Rows are sorted, so a group's entries are one contiguous
 //     segment of every row, located through the row split table (written by the QC pass or
 //     by row_splits_kernel).  CTAs are dealt to groups in proportion to the groups' nnz
 //     (fused_plan_kernel, on the device), rows to a group's CTAs by an atomic cursor.
-//   * Accumulators.  Default: 64-bit FIXED-POINT sums held as two u32 words and updated
-//     with two native 32-bit shared atomics (ATOMS.ADD; the low word's carry-out is added
-//     to the high word), because 64-bit / floating-point shared atomics are CAS loops on
-//     sm_100 (5x slower, measured).  Integer adds commute, so the sums are independent of
-//     the order of the adds.  Scales are powers of two chosen from target_sum so that
-//     4096 rows cannot overflow; a CTA flushes to the global double sums after at most
-//     4096 rows.  Resolution: 2^-48 (S1 log), 2^-44 (S2 log), 2^(E-52) (S1 lin, 2^E >
-//     target_sum); S2 lin uses two windows (x' < 2^(E-10): 2^(2E-72), else 2^(2E-52)), so
-//     every addend keeps >= 31 significant bits.  RSC_MOMENTS_FP64_ACC selects plain
-//     double accumulators (CAS atomics) instead: any value range, slower.
+//   * Segments are walked in 16-byte aligned quads: one 128-bit load per array and one
+//     128-bit store per lane; only the first / last quad of a segment can be partial and
+//     takes scalar accesses.
+//   * Accumulators: EXACT integer sums.  Only 32-bit integer shared atomics are native on
+//     sm_100 (ATOMS.ADD; 64-bit and floating-point ones are CAS loops), so a value v is
+//     first scaled by a power of two 2^k chosen (on the device, from the largest cell
+//     total) such that a = v * 2^k is an exact integer for every v >= 2^(23-k) -- the
+//     float32 significand has 24 bits -- and then
+//         S1 += a      as a 64-bit  integer in two   u32 words (w0, w1)
+//         S2 += a * a  as a 96-bit  integer in three u32 words (s0, s1, s2)
+//     where a word's carry-out (seen in the value the atomic returns) is added to the next
+//     word.  For 2^23 <= a < 2^32 (the usual case: a 512-fold range of v) the upper words
+//     only receive carries: ~3.1 atomics per entry and set.  a >= 2^32 takes the same path
+//     with 64-bit a (a < 2^42 by construction); v below the window (or negative / NaN) goes
+//     to the global double sums directly.  Integer adds commute, so the sums are exact and
+//     independent of the order of the adds; they are converted to double once per flush
+//     (every <= 4092 rows, so no word can overflow).
+//   * RSC_MOMENTS_FP64_ACC selects plain double accumulators (CAS atomics) instead: any
+//     value range, slower (fused_stream_fp64_kernel).
 #include <math.h>
+
+#include <type_traits>
 
 #include "common.cuh"
 
 namespace rsc {
 
 constexpr int kFuThreads = 1024;
-constexpr int kFuUnroll = 4;
 constexpr int kFuRowsPerGrab = 4;
 constexpr int kMaxGroups = 64;
+constexpr int kSetWords = 5;               // u32 words per gene and moment set (w0 w1 s0 s1 s2)
+constexpr int kMaxRangeBits = 19;          // 2^k * v_max <= 2^(23 + 19) = 2^42
 
-struct FusedPlan {            // in the workspace; written by fused_plan_kernel
+struct MomentScale {                       // one per moment set; written by fused_plan_kernel
+  float mult;                              // 2^k
+  float pad;
+  double inv1;                             // 2^-k
+  double inv2;                             // 2^-2k
+};
+
+struct FusedPlan {                         // in the workspace
   int32_t n_groups;
   int32_t pad;
   int32_t cta_first[kMaxGroups + 1];
   unsigned long long row_counter[kMaxGroups];
-};
-
-struct FixedScales {
-  float m_s1log, m_s2log_h, m_s1lin, m_s2hi_h, m_s2lo_h, lin_theta;
-  double inv_s1log, inv_s2log, inv_s1lin, inv_s2hi, inv_s2lo;
+  unsigned long long tmax;                 // largest cell total (fused_tmax_kernel)
+  MomentScale sc_log, sc_lin;
 };
 
 struct FusedArgs {
@@ -51,6 +67,7 @@ struct FusedArgs {
   int32_t n_fine;            // K
   int32_t fine_per_group;
   int32_t Gt;                // accumulator slots per CTA = fine_per_group * RSC_SPLIT_WIDTH
+  int64_t nnz;
   const int64_t* indptr;
   const int32_t* indices;
   float* data;
@@ -58,14 +75,51 @@ struct FusedArgs {
   const uint32_t* splits;
   float target_sum;
   uint32_t row_budget;       // a CTA stops grabbing rows once it has taken this many (then flushes)
-  FixedScales fs;
   double* S1log; double* S2log; double* S1lin; double* S2lin;
   FusedPlan* plan;
 };
 
+// ------------------------------------------------------------------ largest cell total
+__global__ void __launch_bounds__(256)
+fused_tmax_kernel(FusedPlan* plan, int64_t n_rows, const int64_t* __restrict__ cell_total) {
+  long long m = 0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_rows;
+       i += (int64_t)gridDim.x * blockDim.x)
+    m = max(m, (long long)cell_total[i]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(&plan->tmax, (unsigned long long)m);
+}
+
+// floor(log2(x)) for finite x > 0
+__device__ __forceinline__ int floor_log2(double x) {
+  int e;
+  frexp(x, &e);                                            // x = m 2^e, m in [0.5, 1)
+  return e - 1;
+}
+
+__device__ inline MomentScale make_scale(double v_min, double v_max) {
+  // window bottom 2^L <= v_min (so that every expected value converts exactly), but no more
+  // than kMaxRangeBits binades below the top 2^E > v_max
+  int E;
+  frexp(v_max, &E);
+  int L = floor_log2(v_min);
+  if (L < E - kMaxRangeBits) L = E - kMaxRangeBits;
+  if (L > E - 9) L = E - 9;                                // nothing gained by a narrower window
+  int k = 23 - L;
+  if (k > 100) k = 100;
+  if (k < -60) k = -60;
+  MomentScale s;
+  s.mult = (float)ldexp(1.0, k);
+  s.pad = 0.0f;
+  s.inv1 = ldexp(1.0, -k);
+  s.inv2 = ldexp(1.0, -2 * k);
+  return s;
+}
+
 // ------------------------------------------------------------------ plan (1 CTA)
 __global__ void __launch_bounds__(1024)
-fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid,
+fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid, float target_sum,
                   const int32_t* __restrict__ gene_n_cells) {
   __shared__ double mass[kMaxGroups];
   const int tid = threadIdx.x;
@@ -111,28 +165,141 @@ fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid,
     for (int c = 0; c < ng; ++c) { plan->cta_first[c] = acc; acc += n[c]; plan->row_counter[c] = 0ull; }
     plan->cta_first[ng] = acc;
   }
+  if (tid == 32) {
+    // power-of-two scales of the integer accumulators: x' of a unit count in the deepest
+    // cell is target_sum / T_max; nothing exceeds target_sum (non-negative data)
+    const unsigned long long tm = plan->tmax;
+    const double ts = (double)target_sum;
+    const float smin_f = tm != 0ull ? __fdiv_rn(target_sum, (float)(long long)tm) : 1.0f;
+    double smin = (double)smin_f;
+    if (!(smin > 0.0) || !isfinite(smin)) smin = 1.0;
+    if (smin > ts) smin = ts;
+    plan->sc_lin = make_scale(smin, ts);
+    plan->sc_log = make_scale(log1p(smin), log1p(ts) * 1.000001);
+  }
 }
 
 // ------------------------------------------------------------------ accumulator primitives
-// 64-bit add on two u32 words with native shared atomics; exact modulo 2^64 for any
-// interleaving (the carry of the low word is added to the high word by whoever caused it).
-__device__ __forceinline__ void add64(uint32_t* lo, uint32_t* hi, unsigned long long v) {
-  const uint32_t vl = (uint32_t)v, vh = (uint32_t)(v >> 32);
-  const uint32_t old = atomicAdd(lo, vl);
-  atomicAdd(hi, vh + ((old + vl) < old ? 1u : 0u));
+// native 32-bit shared atomics on 32-bit shared addresses
+__device__ __forceinline__ uint32_t atoms_add(uint32_t saddr, uint32_t v) {
+  uint32_t old;
+  asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(saddr), "r"(v));
+  return old;
+}
+__device__ __forceinline__ void reds_add(uint32_t saddr, uint32_t v) {
+  asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(saddr), "r"(v));
 }
 
-template <bool LOG, bool LIN, bool FIXED>
-struct Acc {
-  static constexpr int kLogWords = LOG ? (FIXED ? 4 : 4) : 0;     // u32 words per gene
-  static constexpr int kLinWords = LIN ? (FIXED ? 6 : 4) : 0;
-  static constexpr int kWords = kLogWords + kLinWords;
+// 2^23 <= t < 2^32 (t = v * 2^k): the float is an exact integer that fits one word
+__device__ __forceinline__ bool in_window(float t) {
+  return (__float_as_uint(t) - 0x4B000000u) < 0x04800000u;
+}
+
+// S1 += a, S2 += a * a for a one-word a; sa = shared byte address of the slot's word 0.
+// Three returning atomics (w0, s0, s1) and two predicated carry increments (w1, s2).
+__device__ __forceinline__ void acc_word(uint32_t sa, uint32_t a) {
+  const unsigned long long q = (unsigned long long)a * a;
+  const uint32_t q0 = (uint32_t)q, q1 = (uint32_t)(q >> 32);      // q1 <= 2^32 - 2
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      ".reg .u32 o, t;\n\t"
+      "atom.shared.add.u32 o, [%0], %1;\n\t"
+      "add.u32 t, o, %1;\n\t"
+      "setp.lt.u32 p, t, o;\n\t"
+      "@p red.shared.add.u32 [%0+4], 1;\n\t"
+      "atom.shared.add.u32 o, [%0+8], %2;\n\t"
+      "add.u32 t, o, %2;\n\t"
+      "setp.lt.u32 p, t, o;\n\t"
+      "selp.u32 t, 1, 0, p;\n\t"
+      "add.u32 t, t, %3;\n\t"
+      "atom.shared.add.u32 o, [%0+12], t;\n\t"
+      "add.u32 o, o, t;\n\t"
+      "setp.lt.u32 p, o, t;\n\t"
+      "@p red.shared.add.u32 [%0+16], 1;\n\t"
+      "}"
+      ::"r"(sa), "r"(a), "r"(q0), "r"(q1));
+}
+
+// predicated carry increment of a shared word
+__device__ __forceinline__ void reds_inc_if(uint32_t saddr, bool on) {
+  if (on) asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(saddr));
+}
+
+// acc_word for the 4 entries of a quad, staged so that the returning atomics of the four
+// entries are in flight together (their slots are distinct: one row, four columns)
+__device__ __forceinline__ void acc_quad(uint32_t base, const uint32_t (&so)[4], const uint32_t (&a)[4]) {
+  uint32_t o[4], o0[4], q0[4], q1[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) o[k] = atoms_add(base + so[k], a[k]);
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const unsigned long long q = (unsigned long long)a[k] * a[k];
+    q0[k] = (uint32_t)q; q1[k] = (uint32_t)(q >> 32);             // q1 <= 2^32 - 2
+    o0[k] = atoms_add(base + so[k] + 8, q0[k]);
+  }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) reds_inc_if(base + so[k] + 4, o[k] + a[k] < o[k]);
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    q1[k] += (o0[k] + q0[k] < o0[k]) ? 1u : 0u;
+    o[k] = atoms_add(base + so[k] + 12, q1[k]);
+  }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) reds_inc_if(base + so[k] + 16, o[k] + q1[k] < o[k]);
+}
+
+// any other value: wide a (2^32 <= a < 2^42), or outside the integer window -> global sums
+__device__ __noinline__ void acc_slow(uint32_t sa, float v, float mult, double* S1g, double* S2g) {
+  if (v == 0.0f) return;
+  const float t = v * mult;
+  if (in_window(t)) { acc_word(sa, __float2uint_rz(t)); return; }
+  if (t >= 4294967296.0f && t < 4398046511104.0f) {               // [2^32, 2^42)
+    const unsigned long long a = __float2ull_rz(t);
+    const uint32_t a0 = (uint32_t)a, a1 = (uint32_t)(a >> 32);
+    const uint32_t o = atoms_add(sa, a0);
+    reds_add(sa + 4, a1 + ((o + a0 < o) ? 1u : 0u));
+    const unsigned long long plo = a * a, phi = __umul64hi(a, a);  // phi < 2^20
+    const uint32_t q0 = (uint32_t)plo, q1 = (uint32_t)(plo >> 32), q2 = (uint32_t)phi;
+    const uint32_t o0 = atoms_add(sa + 8, q0);
+    const unsigned long long m = (unsigned long long)q1 + ((o0 + q0 < o0) ? 1u : 0u);
+    const uint32_t m0 = (uint32_t)m;
+    const uint32_t o1 = atoms_add(sa + 12, m0);
+    reds_add(sa + 16, q2 + (uint32_t)(m >> 32) + ((o1 + m0 < o1) ? 1u : 0u));
+    return;
+  }
+  const double d = (double)v;                                      // below the window, negative, NaN
+  atomicAdd(S1g, d);
+  atomicAdd(S2g, d * d);
+}
+
+// what the per-entry code needs to know about the CTA's accumulators
+struct AccCtx {
+  uint32_t sb_log, sb_lin;     // shared byte addresses of the two sets' tables
+  float mult_log, mult_lin;
+  int g0;
+  uint32_t last_slot;          // Gt - 1
+  double *S1log, *S2log, *S1lin, *S2lin;
 };
 
-template <bool LOG, bool LIN, bool FIXED>
+// one entry, any value: normalise, log1p, accumulate; returns x''
+template <bool LOG, bool LIN>
+__device__ __noinline__ float entry_any(const AccCtx& c, int j, float x, float scale) {
+  const float xn = __fmul_rn(x, scale);
+  const float xl = log1p_f32(xn);
+  const uint32_t slot = min((uint32_t)(j - c.g0), c.last_slot);       // stays inside the table
+  if (LOG) acc_slow(c.sb_log + slot * (kSetWords * 4u), xl, c.mult_log, c.S1log + c.g0 + slot,
+                    c.S2log + c.g0 + slot);
+  if (LIN) acc_slow(c.sb_lin + slot * (kSetWords * 4u), xn, c.mult_lin, c.S1lin + c.g0 + slot,
+                    c.S2lin + c.g0 + slot);
+  return xl;
+}
+
+// ------------------------------------------------------------------ streaming kernel
+template <bool LOG, bool LIN>
 __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const FusedArgs a) {
   extern __shared__ __align__(16) uint32_t fsm[];
-  using A = Acc<LOG, LIN, FIXED>;
+  constexpr int kSets = (LOG ? 1 : 0) + (LIN ? 1 : 0);
   __shared__ unsigned s_rows;
   const int tid = threadIdx.x, lane = tid & 31;
   const int Gt = a.Gt;
@@ -145,17 +312,26 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
     const int ng = plan->n_groups;
     while (grp + 1 < ng && (int)blockIdx.x >= plan->cta_first[grp + 1]) ++grp;
   }
+  const float mult_log = plan->sc_log.mult, mult_lin = plan->sc_lin.mult;
   const int f0 = grp * a.fine_per_group;
   const int f1 = min(K, f0 + a.fine_per_group);
   const int g0 = f0 << RSC_SPLIT_SHIFT;
   const int ng_genes = min(a.n_cols, f1 << RSC_SPLIT_SHIFT) - g0;
   unsigned long long* counter = &a.plan->row_counter[grp];
 
-  uint32_t* wlog = fsm;                                   // LOG words: [4][Gt]
-  uint32_t* wlin = fsm + (size_t)A::kLogWords * Gt;       // LIN words: [6 or 4][Gt]
-  for (int i = tid; i < A::kWords * Gt; i += kFuThreads) fsm[i] = 0u;
-
-  const FixedScales fs = a.fs;
+  // set s of slot g lives at fsm[(s * Gt + g) * 5 .. + 5): a stride of 5 words is odd, so the
+  // slots of a warp spread over all 32 banks
+  AccCtx cx;
+  {
+    uint32_t sb = (uint32_t)__cvta_generic_to_shared(fsm);
+    asm volatile("mov.u32 %0, %0;" : "+r"(sb));           // keep it in a register (no recomputation)
+    cx.sb_log = sb;
+    cx.sb_lin = sb + (LOG ? (uint32_t)Gt * (kSetWords * 4u) : 0u);
+  }
+  cx.mult_log = mult_log; cx.mult_lin = mult_lin; cx.g0 = g0; cx.last_slot = (uint32_t)(Gt - 1);
+  cx.S1log = a.S1log; cx.S2log = a.S2log; cx.S1lin = a.S1lin; cx.S2lin = a.S2lin;
+  const uint32_t sb_log = cx.sb_log, sb_lin = cx.sb_lin, last_slot = cx.last_slot;
+  for (int i = tid; i < kSets * kSetWords * Gt + kSetWords; i += kFuThreads) fsm[i] = 0u;
 
   auto grab_issue = [&]() -> long long {                  // lane 0 only holds the result
     long long r = -1;
@@ -164,6 +340,46 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
       if (c < a.row_budget) r = (long long)atomicAdd(counter, (unsigned long long)kFuRowsPerGrab);
     }
     return r;
+  };
+
+  // One quad of 4 consecutive entries.  Straight-line code when every value is in the usual
+  // range (x' >= 0.25 and inside the integer windows), else entry by entry through entry_any.
+  // EDGE: only entries e0 + k in [0, len) belong to the segment; the others (a neighbouring
+  // segment's) are neutralised by adding 0 to the spare slot Gt, so the code stays branch-free.
+  auto quad = [&](auto edge_tag, const int4 jv, const float4 xv, float scale, int e0, int len) -> float4 {
+    constexpr bool EDGE = decltype(edge_tag)::value;
+    const int j[4] = {jv.x, jv.y, jv.z, jv.w};
+    const float x[4] = {xv.x, xv.y, xv.z, xv.w};
+    float xn[4], xl[4], tl[4], tn[4];
+    bool valid[4];
+    bool ok = true;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      valid[k] = !EDGE || (unsigned)(e0 + k) < (unsigned)len;
+      xn[k] = __fmul_rn(x[k], scale);
+      xl[k] = log1p_ge_quarter(xn[k]);
+      bool okk = xn[k] >= 0.25f;
+      if (LOG) { tl[k] = xl[k] * mult_log; okk = okk && in_window(tl[k]); }
+      if (LIN) { tn[k] = xn[k] * mult_lin; okk = okk && in_window(tn[k]); }
+      ok = ok && (okk || !valid[k]);
+    }
+    if (ok) {
+      uint32_t so[4], al[4], an[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const uint32_t slot = valid[k] ? min((uint32_t)(j[k] - g0), last_slot) : (uint32_t)Gt;
+        so[k] = slot * (kSetWords * 4u);
+        if (LOG) al[k] = valid[k] ? __float2uint_rz(tl[k]) : 0u;
+        if (LIN) an[k] = valid[k] ? __float2uint_rz(tn[k]) : 0u;
+      }
+      if (LOG) acc_quad(sb_log, so, al);
+      if (LIN) acc_quad(sb_lin, so, an);
+    } else {
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (valid[k]) xl[k] = entry_any<LOG, LIN>(cx, j[k], x[k], scale);
+    }
+    return make_float4(xl[0], xl[1], xl[2], xl[3]);
   };
 
   int done;
@@ -188,56 +404,79 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
           mscale = cell_scale(a.target_sum, a.cell_total[row]);
         }
       }
-#pragma unroll 1
-      for (int ri = 0; ri < kFuRowsPerGrab; ++ri) {
+      // The grab's segments are walked in steps of 32 quads (one per lane); the loads of step
+      // i + 1 are issued before step i is computed (software pipeline, one step deep).
+      struct Seg { int64_t abeg; int head, len, nq; float scale; };
+      auto seg_of = [&](int ri) -> Seg {                  // warp-uniform; ri < kFuRowsPerGrab
         const int64_t beg = __shfl_sync(0xffffffffu, mbeg, ri);
         const int64_t end = __shfl_sync(0xffffffffu, mend, ri);
-        const float scale = __shfl_sync(0xffffffffu, mscale, ri);
-        for (int64_t base = beg; base < end; base += 32 * kFuUnroll) {
-          int j[kFuUnroll];
-          float x[kFuUnroll];
-#pragma unroll
-          for (int u = 0; u < kFuUnroll; ++u) {
-            const int64_t p = base + u * 32 + lane;
-            const bool ok = p < end;
-            j[u] = ok ? __ldg(a.indices + p) : -1;
-            x[u] = ok ? a.data[p] : 0.0f;
+        Seg s;
+        s.scale = __shfl_sync(0xffffffffu, mscale, ri);
+        s.abeg = beg & ~3LL;
+        s.head = (int)(beg - s.abeg);
+        s.len = end > beg ? (int)(end - beg) : 0;
+        s.nq = s.len > 0 ? (s.head + s.len + 3) >> 2 : 0;
+        return s;
+      };
+      auto load_step = [&](const Seg& s, int q0, int4& jv, float4& xv) {
+        const int q = q0 + lane;
+        if (q >= s.nq) return;
+        const int64_t off = s.abeg + 4LL * q;
+        if (off + 4 <= a.nnz) {
+          jv = __ldg(reinterpret_cast<const int4*>(a.indices + off));
+          xv = *reinterpret_cast<const float4*>(a.data + off);
+        } else {                                          // the last quad of the whole matrix
+          const int e0 = q * 4 - s.head;
+          jv = make_int4(0, 0, 0, 0);
+          xv = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (e0 + 0 < s.len) { jv.x = __ldg(a.indices + off + 0); xv.x = a.data[off + 0]; }
+          if (e0 + 1 < s.len) { jv.y = __ldg(a.indices + off + 1); xv.y = a.data[off + 1]; }
+          if (e0 + 2 < s.len) { jv.z = __ldg(a.indices + off + 2); xv.z = a.data[off + 2]; }
+        }
+      };
+      auto compute_step = [&](const Seg& s, int q0, const int4& jv, const float4& xv) {
+        const int q = q0 + lane;
+        const int e0 = q * 4 - s.head;
+        const bool full = e0 >= 0 && e0 + 4 <= s.len;
+        float* dq = a.data + s.abeg + 4LL * q;
+        if (__all_sync(0xffffffffu, full)) {
+          *reinterpret_cast<float4*>(dq) = quad(std::false_type{}, jv, xv, s.scale, e0, s.len);
+        } else if (q < s.nq) {
+          const float4 r = quad(std::true_type{}, jv, xv, s.scale, e0, s.len);
+          if (full) {
+            *reinterpret_cast<float4*>(dq) = r;
+          } else {
+            if ((unsigned)(e0 + 0) < (unsigned)s.len) dq[0] = r.x;
+            if ((unsigned)(e0 + 1) < (unsigned)s.len) dq[1] = r.y;
+            if ((unsigned)(e0 + 2) < (unsigned)s.len) dq[2] = r.z;
+            if ((unsigned)(e0 + 3) < (unsigned)s.len) dq[3] = r.w;
           }
-#pragma unroll
-          for (int u = 0; u < kFuUnroll; ++u) {
-            const int slot = j[u] - g0;
-            if (j[u] >= 0 && (unsigned)slot < (unsigned)Gt) {
-              const float xn = __fmul_rn(x[u], scale);
-              const float xl = log1p_f32(xn);
-              a.data[base + u * 32 + lane] = xl;
-              if (FIXED) {
-                if (LOG) {
-                  add64(wlog + slot, wlog + Gt + slot, __float2ull_rn(xl * fs.m_s1log));
-                  const double d = (double)(xl * fs.m_s2log_h);
-                  add64(wlog + 2 * Gt + slot, wlog + 3 * Gt + slot, __double2ull_rn(d * d));
-                }
-                if (LIN) {
-                  add64(wlin + slot, wlin + Gt + slot, __float2ull_rn(xn * fs.m_s1lin));
-                  const bool small = xn < fs.lin_theta;
-                  const double d = (double)(xn * (small ? fs.m_s2lo_h : fs.m_s2hi_h));
-                  uint32_t* w = wlin + (small ? 4 : 2) * Gt + slot;
-                  add64(w, w + Gt, __double2ull_rn(d * d));
-                }
-              } else {
-                if (LOG) {
-                  double* t = reinterpret_cast<double*>(wlog);
-                  const double v = (double)xl;
-                  atomicAdd(t + slot, v);
-                  atomicAdd(t + Gt + slot, v * v);
-                }
-                if (LIN) {
-                  double* t = reinterpret_cast<double*>(wlin);
-                  const double v = (double)xn;
-                  atomicAdd(t + slot, v);
-                  atomicAdd(t + Gt + slot, v * v);
-                }
-              }
+        }
+      };
+      {
+        int ri = 0;
+        Seg S = seg_of(0);
+        while (S.nq == 0 && ++ri < kFuRowsPerGrab) S = seg_of(ri);
+        if (ri < kFuRowsPerGrab) {
+          int q0 = 0;
+          int4 jc = make_int4(0, 0, 0, 0);
+          float4 xc = make_float4(0.f, 0.f, 0.f, 0.f);
+          load_step(S, q0, jc, xc);
+          for (;;) {
+            Seg N = S;
+            int nq0 = q0 + 32, nri = ri;
+            if (nq0 >= S.nq) {
+              nq0 = 0;
+              N.nq = 0;
+              while (++nri < kFuRowsPerGrab) { N = seg_of(nri); if (N.nq) break; }
             }
+            const bool has_next = nri < kFuRowsPerGrab;
+            int4 jn = make_int4(0, 0, 0, 0);
+            float4 xn4 = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (has_next) load_step(N, nq0, jn, xn4);
+            compute_step(S, q0, jc, xc);
+            if (!has_next) break;
+            S = N; q0 = nq0; ri = nri; jc = jn; xc = xn4;
           }
         }
       }
@@ -247,42 +486,92 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
     // flush this CTA's accumulators into the global double sums and clear them
     for (int s = tid; s < ng_genes; s += kFuThreads) {
       const int g = g0 + s;
-      if (FIXED) {
-        if (LOG) {
-          const unsigned long long v1 = ((unsigned long long)wlog[Gt + s] << 32) | wlog[s];
-          const unsigned long long v2 = ((unsigned long long)wlog[3 * Gt + s] << 32) | wlog[2 * Gt + s];
-          if (v1 | v2) {
-            atomicAdd(&a.S1log[g], (double)v1 * fs.inv_s1log);
-            atomicAdd(&a.S2log[g], (double)v2 * fs.inv_s2log);
-            wlog[s] = 0u; wlog[Gt + s] = 0u; wlog[2 * Gt + s] = 0u; wlog[3 * Gt + s] = 0u;
-          }
+#pragma unroll
+      for (int set = 0; set < kSets; ++set) {
+        const bool is_log = LOG && set == 0;
+        uint32_t* w = fsm + ((size_t)set * Gt + s) * kSetWords;
+        const uint32_t w0 = w[0], w1 = w[1], s0 = w[2], s1 = w[3], s2 = w[4];
+        if (w0 | w1 | s0 | s1 | s2) {
+          const MomentScale& sc = is_log ? plan->sc_log : plan->sc_lin;
+          const double v1 = (double)(((unsigned long long)w1 << 32) | w0) * sc.inv1;
+          const double v2 = ((double)s2 * 18446744073709551616.0 +
+                             (double)(((unsigned long long)s1 << 32) | s0)) * sc.inv2;
+          atomicAdd(is_log ? &a.S1log[g] : &a.S1lin[g], v1);
+          atomicAdd(is_log ? &a.S2log[g] : &a.S2lin[g], v2);
+          w[0] = 0u; w[1] = 0u; w[2] = 0u; w[3] = 0u; w[4] = 0u;
         }
-        if (LIN) {
-          const unsigned long long v1 = ((unsigned long long)wlin[Gt + s] << 32) | wlin[s];
-          const unsigned long long vh = ((unsigned long long)wlin[3 * Gt + s] << 32) | wlin[2 * Gt + s];
-          const unsigned long long vl = ((unsigned long long)wlin[5 * Gt + s] << 32) | wlin[4 * Gt + s];
-          if (v1 | vh | vl) {
-            atomicAdd(&a.S1lin[g], (double)v1 * fs.inv_s1lin);
-            atomicAdd(&a.S2lin[g], (double)vh * fs.inv_s2hi + (double)vl * fs.inv_s2lo);
-            wlin[s] = 0u; wlin[Gt + s] = 0u; wlin[2 * Gt + s] = 0u; wlin[3 * Gt + s] = 0u;
-            wlin[4 * Gt + s] = 0u; wlin[5 * Gt + s] = 0u;
-          }
+      }
+    }
+  } while (!done);
+}
+
+// ------------------------------------------------------------------ double accumulators
+// RSC_MOMENTS_FP64_ACC: per-gene doubles in shared memory, CAS atomics; any value range.
+template <bool LOG, bool LIN>
+__global__ void __launch_bounds__(kFuThreads, 1) fused_stream_fp64_kernel(const FusedArgs a) {
+  extern __shared__ __align__(16) uint32_t fsm[];
+  __shared__ unsigned s_rows;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int Gt = a.Gt;
+  const int K = a.n_fine;
+  const FusedPlan* plan = a.plan;
+  int grp = 0;
+  {
+    const int ng = plan->n_groups;
+    while (grp + 1 < ng && (int)blockIdx.x >= plan->cta_first[grp + 1]) ++grp;
+  }
+  const int f0 = grp * a.fine_per_group;
+  const int f1 = min(K, f0 + a.fine_per_group);
+  const int g0 = f0 << RSC_SPLIT_SHIFT;
+  const int ng_genes = min(a.n_cols, f1 << RSC_SPLIT_SHIFT) - g0;
+  unsigned long long* counter = &a.plan->row_counter[grp];
+  double* tlog = reinterpret_cast<double*>(fsm);                    // [2][Gt]
+  double* tlin = tlog + (LOG ? 2 * (size_t)Gt : 0);                 // [2][Gt]
+  constexpr int kSets = (LOG ? 1 : 0) + (LIN ? 1 : 0);
+  for (int i = tid; i < kSets * 2 * Gt; i += kFuThreads) tlog[i] = 0.0;
+
+  int done;
+  do {
+    if (tid == 0) s_rows = 0u;
+    __syncthreads();
+    int saw_end = 0;
+    for (;;) {
+      long long r0 = -1;
+      if (lane == 0) {
+        const unsigned c = atomicAdd(&s_rows, (unsigned)kFuRowsPerGrab);
+        if (c < a.row_budget) r0 = (long long)atomicAdd(counter, (unsigned long long)kFuRowsPerGrab);
+      }
+      r0 = __shfl_sync(0xffffffffu, r0, 0);
+      if (r0 < 0) break;
+      if (r0 >= a.n_rows) { saw_end = 1; break; }
+      const int nr = (int)min((long long)kFuRowsPerGrab, a.n_rows - r0);
+      for (int ri = 0; ri < nr; ++ri) {
+        const long long row = r0 + ri;
+        const uint32_t* sp = a.splits + (size_t)row * (size_t)(K + 1);
+        const int64_t rb = a.indptr[row];
+        const int64_t beg = rb + sp[f0], end = rb + sp[f1];
+        const float scale = cell_scale(a.target_sum, a.cell_total[row]);
+        for (int64_t p = beg + lane; p < end; p += 32) {
+          const int slot = __ldg(a.indices + p) - g0;
+          const float xn = __fmul_rn(a.data[p], scale);
+          const float xl = log1p_f32(xn);
+          a.data[p] = xl;
+          if ((unsigned)slot >= (unsigned)Gt) continue;
+          if (LOG) { const double v = (double)xl; atomicAdd(tlog + slot, v); atomicAdd(tlog + Gt + slot, v * v); }
+          if (LIN) { const double v = (double)xn; atomicAdd(tlin + slot, v); atomicAdd(tlin + Gt + slot, v * v); }
         }
-      } else {
-        if (LOG) {
-          double* t = reinterpret_cast<double*>(wlog);
-          if (t[s] != 0.0 || t[Gt + s] != 0.0) {
-            atomicAdd(&a.S1log[g], t[s]); atomicAdd(&a.S2log[g], t[Gt + s]);
-            t[s] = 0.0; t[Gt + s] = 0.0;
-          }
-        }
-        if (LIN) {
-          double* t = reinterpret_cast<double*>(wlin);
-          if (t[s] != 0.0 || t[Gt + s] != 0.0) {
-            atomicAdd(&a.S1lin[g], t[s]); atomicAdd(&a.S2lin[g], t[Gt + s]);
-            t[s] = 0.0; t[Gt + s] = 0.0;
-          }
-        }
+      }
+    }
+    done = __syncthreads_or(saw_end);
+    for (int s = tid; s < ng_genes; s += kFuThreads) {
+      const int g = g0 + s;
+      if (LOG && (tlog[s] != 0.0 || tlog[Gt + s] != 0.0)) {
+        atomicAdd(&a.S1log[g], tlog[s]); atomicAdd(&a.S2log[g], tlog[Gt + s]);
+        tlog[s] = 0.0; tlog[Gt + s] = 0.0;
+      }
+      if (LIN && (tlin[s] != 0.0 || tlin[Gt + s] != 0.0)) {
+        atomicAdd(&a.S1lin[g], tlin[s]); atomicAdd(&a.S2lin[g], tlin[Gt + s]);
+        tlin[s] = 0.0; tlin[Gt + s] = 0.0;
       }
     }
   } while (!done);
@@ -294,21 +583,30 @@ int launch_fused_generic(const rsc_csr&, float, const int64_t*, int, double*, do
 
 static int fused_grid() { return g_opt.grid_ctas > 0 ? g_opt.grid_ctas : sm_count(); }
 
-static int words_per_gene(int which, bool fixed) {
-  int w = 0;
-  if (which & RSC_MOMENTS_LOG) w += 4;
-  if (which & RSC_MOMENTS_LIN) w += fixed ? 6 : 4;
-  return w;
+// bytes of shared-memory accumulators per gene
+static int bytes_per_gene(int which) {
+  const int sets = ((which & RSC_MOMENTS_LOG) ? 1 : 0) + ((which & RSC_MOMENTS_LIN) ? 1 : 0);
+  return sets * ((which & RSC_MOMENTS_FP64_ACC) ? 16 : kSetWords * 4);
+}
+
+// column blocks per group: as many as fit, then evened out over the groups
+static int fine_per_group(int32_t n_cols, int which) {
+  const int bpg = bytes_per_gene(which);
+  if (bpg == 0) return 0;
+  const int fit = (int)((kMaxDynSmem - 64) / ((size_t)bpg * RSC_SPLIT_WIDTH));
+  if (fit < 1) return 0;
+  const int K = split_blocks(n_cols);
+  const int ng = (K + fit - 1) / fit;
+  return (K + ng - 1) / ng;
 }
 
 // true when the streaming kernel can serve this call (else: generic L2-atomic kernel)
-static bool fused_fast_ok(const rsc_csr& X, float target_sum, int which) {
+static bool fused_fast_ok(const rsc_csr& X, int which) {
   if (!(X.flags & RSC_CSR_SORTED) || g_opt.force_generic) return false;
   if ((which & 3) == 0) return false;
-  const bool fixed = !(which & RSC_MOMENTS_FP64_ACC);
-  if (fixed && !(target_sum < 1.0e9f)) return false;
-  const int wpg = words_per_gene(which, fixed);
-  const int fpg = (int)((kMaxDynSmem - 64) / ((size_t)wpg * 4 * RSC_SPLIT_WIDTH));
+  // 128-bit accesses need 16-byte aligned arrays
+  if ((reinterpret_cast<uintptr_t>(X.indices) | reinterpret_cast<uintptr_t>(X.data)) & 15) return false;
+  const int fpg = fine_per_group(X.n_cols, which);
   if (fpg < 1) return false;
   const int K = split_blocks(X.n_cols);
   const int ng = (K + fpg - 1) / fpg;
@@ -321,39 +619,10 @@ size_t fused_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t) {
          align_up(sizeof(uint32_t) * (size_t)n_rows * K1, 256);
 }
 
-static FixedScales make_scales(float target_sum) {
-  // 2^E > target_sum >= x' ;  2^EL > log1p(target_sum) >= x''
-  int E = 0, EL = 0;
-  frexp((double)target_sum, &E);                           // target_sum = m 2^E, m in [0.5, 1)
-  frexp(log1p((double)target_sum) * 1.000001, &EL);
-  if (E < 1) E = 1;
-  if (EL < 1) EL = 1;
-  FixedScales s;
-  const int k1log = 52 - EL, k2log = 52 - 2 * EL, k1lin = 52 - E, k2hi = 52 - 2 * E,
-            k2lo = 72 - 2 * E;
-  s.m_s1log = (float)ldexp(1.0, k1log);
-  s.m_s2log_h = (float)ldexp(1.0, k2log / 2);
-  s.m_s1lin = (float)ldexp(1.0, k1lin);
-  s.m_s2hi_h = (float)ldexp(1.0, k2hi / 2);
-  s.m_s2lo_h = (float)ldexp(1.0, k2lo / 2);
-  s.lin_theta = (float)ldexp(1.0, E - 10);
-  s.inv_s1log = ldexp(1.0, -k1log);
-  s.inv_s2log = ldexp(1.0, -k2log);
-  s.inv_s1lin = ldexp(1.0, -k1lin);
-  s.inv_s2hi = ldexp(1.0, -k2hi);
-  s.inv_s2lo = ldexp(1.0, -k2lo);
-  return s;
-}
-
-template <bool LOG, bool LIN, bool FIXED>
-static int launch_stream(const FusedArgs& a, size_t smem, cudaStream_t st) {
-  static bool attr_set = false;
-  if (!attr_set) {
-    RSC_CUDA(cudaFuncSetAttribute(fused_stream_kernel<LOG, LIN, FIXED>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem));
-    attr_set = true;
-  }
-  fused_stream_kernel<LOG, LIN, FIXED><<<fused_grid(), kFuThreads, smem, st>>>(a);
+template <typename Kern>
+static int launch_stream(Kern kern, const FusedArgs& a, size_t smem, cudaStream_t st) {
+  RSC_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem));
+  kern<<<fused_grid(), kFuThreads, smem, st>>>(a);
   RSC_LAUNCH_CHECK("fused_stream_kernel");
   return RSC_OK;
 }
@@ -370,11 +639,10 @@ int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i
   double* S1lin = sums_out ? sums_out + 2 * G : reinterpret_cast<double*>(w + 2 * gsz);
   double* S2lin = sums_out ? sums_out + 3 * G : reinterpret_cast<double*>(w + 3 * gsz);
   int rc;
-  if (!fused_fast_ok(X, target_sum, which) || X.n_rows == 0) {
+  if (!fused_fast_ok(X, which) || X.n_rows == 0) {
     rc = launch_fused_generic(X, target_sum, cell_total_i64, which, S1log, S2log, S1lin, S2lin, st);
     if (rc != RSC_OK) return rc;
   } else {
-    const bool fixed = !(which & RSC_MOMENTS_FP64_ACC);
     if (which & RSC_MOMENTS_LOG) {
       RSC_CUDA(cudaMemsetAsync(S1log, 0, sizeof(double) * G, st));
       RSC_CUDA(cudaMemsetAsync(S2log, 0, sizeof(double) * G, st));
@@ -389,27 +657,33 @@ int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i
       if ((rc = launch_row_splits(X, sp, st)) != RSC_OK) return rc;
       row_splits = sp;
     }
-    const int wpg = words_per_gene(which, fixed);
     FusedArgs a;
-    a.n_rows = X.n_rows; a.n_cols = X.n_cols; a.n_fine = split_blocks(X.n_cols);
-    a.fine_per_group = (int)((kMaxDynSmem - 64) / ((size_t)wpg * 4 * RSC_SPLIT_WIDTH));
-    if (a.fine_per_group > a.n_fine) a.fine_per_group = a.n_fine;
+    a.n_rows = X.n_rows; a.n_cols = X.n_cols; a.nnz = X.nnz; a.n_fine = split_blocks(X.n_cols);
+    a.fine_per_group = fine_per_group(X.n_cols, which);
     a.Gt = a.fine_per_group * RSC_SPLIT_WIDTH;
     a.indptr = X.indptr; a.indices = X.indices; a.data = X.data; a.cell_total = cell_total_i64;
-    a.splits = row_splits; a.target_sum = target_sum; a.fs = make_scales(target_sum);
+    a.splits = row_splits; a.target_sum = target_sum;
     a.row_budget = (uint32_t)g_opt.fused_row_budget;
     a.S1log = S1log; a.S2log = S2log; a.S1lin = S1lin; a.S2lin = S2lin; a.plan = plan;
+    RSC_CUDA(cudaMemsetAsync(&plan->tmax, 0, sizeof(unsigned long long), st));
+    {
+      int64_t blocks = (X.n_rows + 255) / 256;
+      const int64_t cap = (int64_t)sm_count() * 4;
+      if (blocks > cap) blocks = cap;
+      fused_tmax_kernel<<<(unsigned)blocks, 256, 0, st>>>(plan, X.n_rows, cell_total_i64);
+      RSC_LAUNCH_CHECK("fused_tmax_kernel");
+    }
     fused_plan_kernel<<<1, 1024, 0, st>>>(plan, X.n_cols, a.n_fine, a.fine_per_group, fused_grid(),
-                                          gene_n_cells);
+                                          target_sum, gene_n_cells);
     RSC_LAUNCH_CHECK("fused_plan_kernel");
-    const size_t smem = (size_t)wpg * 4 * (size_t)a.Gt;
-    switch ((which & 3) | (fixed ? 4 : 0)) {
-      case 1: rc = launch_stream<true, false, false>(a, smem, st); break;
-      case 2: rc = launch_stream<false, true, false>(a, smem, st); break;
-      case 3: rc = launch_stream<true, true, false>(a, smem, st); break;
-      case 5: rc = launch_stream<true, false, true>(a, smem, st); break;
-      case 6: rc = launch_stream<false, true, true>(a, smem, st); break;
-      default: rc = launch_stream<true, true, true>(a, smem, st); break;
+    const size_t smem = (size_t)bytes_per_gene(which) * (size_t)a.Gt + 32;   // + the spare slot
+    switch (which & 7) {
+      case 1: rc = launch_stream(fused_stream_kernel<true, false>, a, smem, st); break;
+      case 2: rc = launch_stream(fused_stream_kernel<false, true>, a, smem, st); break;
+      case 3: rc = launch_stream(fused_stream_kernel<true, true>, a, smem, st); break;
+      case 5: rc = launch_stream(fused_stream_fp64_kernel<true, false>, a, smem, st); break;
+      case 6: rc = launch_stream(fused_stream_fp64_kernel<false, true>, a, smem, st); break;
+      default: rc = launch_stream(fused_stream_fp64_kernel<true, true>, a, smem, st); break;
     }
     if (rc != RSC_OK) return rc;
   }
