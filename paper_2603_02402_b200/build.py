@@ -39,6 +39,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc] + NVCC_FLAGS + ["-I", os.path.join(ROOT, "include"), "-I", CSRC]
+    cmd += os.environ.get("RSC_NVCC_EXTRA", "").split()   # extra nvcc flags (experiments)
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += _sources() + ["-o", LIB, "-lcudart"]

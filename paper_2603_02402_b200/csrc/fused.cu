@@ -39,7 +39,10 @@
 
 namespace rsc {
 
-constexpr int kFuThreads = 1024;
+#ifndef RSC_FU_THREADS
+#define RSC_FU_THREADS 768
+#endif
+constexpr int kFuThreads = RSC_FU_THREADS;
 constexpr int kFuRowsPerGrab = 4;
 constexpr int kMaxGroups = 64;
 constexpr int kSetWords = 5;               // u32 words per gene and moment set (w0 w1 s0 s1 s2)
@@ -226,27 +229,60 @@ __device__ __forceinline__ void reds_inc_if(uint32_t saddr, bool on) {
   if (on) asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(saddr));
 }
 
+// carry-out (0 / 1) of o + v
+__device__ __forceinline__ uint32_t carry_of(uint32_t o, uint32_t v) {
+  uint32_t c;
+  asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\taddc.u32 %0, 0, 0;\n\t}" : "=r"(c) : "r"(o), "r"(v));
+  return c;
+}
+// w + carry-out of (o + v)
+__device__ __forceinline__ uint32_t add_carry_of(uint32_t w, uint32_t o, uint32_t v) {
+  uint32_t r;
+  asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\taddc.u32 %0, %3, 0;\n\t}"
+      : "=r"(r) : "r"(o), "r"(v), "r"(w));
+  return r;
+}
+
 // acc_word for the 4 entries of a quad, staged so that the returning atomics of the four
 // entries are in flight together (their slots are distinct: one row, four columns)
 __device__ __forceinline__ void acc_quad(uint32_t base, const uint32_t (&so)[4], const uint32_t (&a)[4]) {
-  uint32_t o[4], o0[4], q0[4], q1[4];
-#pragma unroll
-  for (int k = 0; k < 4; ++k) o[k] = atoms_add(base + so[k], a[k]);
+  uint32_t sa[4], o[4], o0[4], q0[4], q1[4];
+#if defined(RSC_EXP) && RSC_EXP == 2
+  return;
+#endif
+#if defined(RSC_EXP) && RSC_EXP == 3
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
-    const unsigned long long q = (unsigned long long)a[k] * a[k];
+    sa[k] = base + so[k];
+    unsigned long long q;
+    asm("mul.wide.u32 %0, %1, %1;" : "=l"(q) : "r"(a[k]));
+    reds_add(sa[k], a[k]); reds_add(sa[k] + 8, (uint32_t)q); reds_add(sa[k] + 12, (uint32_t)(q >> 32));
+  }
+  return;
+#endif
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { sa[k] = base + so[k]; o[k] = atoms_add(sa[k], a[k]); }
+#if defined(RSC_EXP) && RSC_EXP == 1
+#pragma unroll
+  for (int k = 0; k < 4; ++k) reds_inc_if(sa[k] + 4, carry_of(o[k], a[k]) != 0u);
+  return;
+#endif
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    unsigned long long q;
+    asm("mul.wide.u32 %0, %1, %1;" : "=l"(q) : "r"(a[k]));
     q0[k] = (uint32_t)q; q1[k] = (uint32_t)(q >> 32);             // q1 <= 2^32 - 2
-    o0[k] = atoms_add(base + so[k] + 8, q0[k]);
+    o0[k] = atoms_add(sa[k] + 8, q0[k]);
   }
 #pragma unroll
-  for (int k = 0; k < 4; ++k) reds_inc_if(base + so[k] + 4, o[k] + a[k] < o[k]);
+  for (int k = 0; k < 4; ++k) reds_inc_if(sa[k] + 4, carry_of(o[k], a[k]) != 0u);
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
-    q1[k] += (o0[k] + q0[k] < o0[k]) ? 1u : 0u;
-    o[k] = atoms_add(base + so[k] + 12, q1[k]);
+    q1[k] = add_carry_of(q1[k], o0[k], q0[k]);
+    o[k] = atoms_add(sa[k] + 12, q1[k]);
   }
 #pragma unroll
-  for (int k = 0; k < 4; ++k) reds_inc_if(base + so[k] + 16, o[k] + q1[k] < o[k]);
+  for (int k = 0; k < 4; ++k) reds_inc_if(sa[k] + 16, carry_of(o[k], q1[k]) != 0u);
 }
 
 // any other value: wide a (2^32 <= a < 2^42), or outside the integer window -> global sums
@@ -387,25 +423,43 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
     if (tid == 0) s_rows = 0u;
     __syncthreads();
     int saw_end = 0;
+    // Grabs are pipelined two deep: while grab g is processed, the row range of grab g + 1 is
+    // already known, its row metadata is loaded and its segments are prefetched into L2, and
+    // the atomic for grab g + 2 is in flight -- no latency chain between grabs.
+    auto load_meta = [&](long long g0row, int64_t& mb, int64_t& me, float& ms) {
+      mb = 0; me = 0; ms = 1.0f;
+      const long long row = g0row + lane;                 // lanes 0..RG-1: one row each
+      if (lane < kFuRowsPerGrab && row < a.n_rows) {
+        const uint32_t* sp = a.splits + (size_t)row * (size_t)(K + 1);
+        const int64_t rb = a.indptr[row];
+        mb = rb + sp[f0];
+        me = rb + sp[f1];
+        ms = cell_scale(a.target_sum, a.cell_total[row]);
+      }
+    };
+    auto l2_prefetch = [&](int64_t mb, int64_t me, int ri) {   // the 128-byte lines of one segment
+      const int64_t pb = __shfl_sync(0xffffffffu, mb, ri);
+      const int64_t pe = __shfl_sync(0xffffffffu, me, ri);
+      for (int64_t p = (pb & ~31LL) + lane * 32; p < pe; p += 32 * 32) {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(a.indices + p));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(a.data + p));
+      }
+    };
     long long r0 = __shfl_sync(0xffffffffu, grab_issue(), 0);
+    int64_t mbeg = 0, mend = 0;
+    float mscale = 1.0f;
+    if (r0 >= 0 && r0 < a.n_rows) load_meta(r0, mbeg, mend, mscale);
+    long long rnext = __shfl_sync(0xffffffffu, grab_issue(), 0);
     while (r0 >= 0) {
       if (r0 >= a.n_rows) { saw_end = 1; break; }
-      const long long pending = grab_issue();             // consumed after this batch of rows
-      // lanes 0..RG-1 fetch the segment bounds and the scale of one row each
-      int64_t mbeg = 0, mend = 0;
-      float mscale = 1.0f;
-      {
-        const long long row = r0 + lane;
-        if (lane < kFuRowsPerGrab && row < a.n_rows) {
-          const uint32_t* sp = a.splits + (size_t)row * (size_t)(K + 1);
-          const int64_t rb = a.indptr[row];
-          mbeg = rb + sp[f0];
-          mend = rb + sp[f1];
-          mscale = cell_scale(a.target_sum, a.cell_total[row]);
-        }
-      }
+      const long long pending = grab_issue();             // grab g + 2; consumed after this grab
+      const bool next_ok = rnext >= 0 && rnext < a.n_rows;
+      int64_t nbeg = 0, nend = 0;
+      float nscale = 1.0f;
+      if (next_ok) load_meta(rnext, nbeg, nend, nscale);
       // The grab's segments are walked in steps of 32 quads (one per lane); the loads of step
-      // i + 1 are issued before step i is computed (software pipeline, one step deep).
+      // i + 1 are issued before step i is computed (software pipeline, one step deep).  A step
+      // is "interior" when all of its 32 quads lie wholly inside the segment: no masks at all.
       struct Seg { int64_t abeg; int head, len, nq; float scale; };
       auto seg_of = [&](int ri) -> Seg {                  // warp-uniform; ri < kFuRowsPerGrab
         const int64_t beg = __shfl_sync(0xffffffffu, mbeg, ri);
@@ -418,32 +472,38 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
         s.nq = s.len > 0 ? (s.head + s.len + 3) >> 2 : 0;
         return s;
       };
-      auto load_step = [&](const Seg& s, int q0, int4& jv, float4& xv) {
-        const int q = q0 + lane;
-        if (q >= s.nq) return;
-        const int64_t off = s.abeg + 4LL * q;
-        if (off + 4 <= a.nnz) {
+      auto interior = [&](const Seg& s, int st) -> bool {
+        return (st > 0 || s.head == 0) && (st * 128 + 128 <= s.head + s.len);
+      };
+      auto load_step = [&](const Seg& s, int st, int4& jv, float4& xv) {
+        const int q = st * 32 + lane;
+        const int64_t off = s.abeg + 4 * q;
+        if (interior(s, st)) {
           jv = __ldg(reinterpret_cast<const int4*>(a.indices + off));
           xv = *reinterpret_cast<const float4*>(a.data + off);
-        } else {                                          // the last quad of the whole matrix
-          const int e0 = q * 4 - s.head;
-          jv = make_int4(0, 0, 0, 0);
-          xv = make_float4(0.f, 0.f, 0.f, 0.f);
-          if (e0 + 0 < s.len) { jv.x = __ldg(a.indices + off + 0); xv.x = a.data[off + 0]; }
-          if (e0 + 1 < s.len) { jv.y = __ldg(a.indices + off + 1); xv.y = a.data[off + 1]; }
-          if (e0 + 2 < s.len) { jv.z = __ldg(a.indices + off + 2); xv.z = a.data[off + 2]; }
+        } else if (q < s.nq) {
+          if (off + 4 <= a.nnz) {
+            jv = __ldg(reinterpret_cast<const int4*>(a.indices + off));
+            xv = *reinterpret_cast<const float4*>(a.data + off);
+          } else {                                        // the last quad of the whole matrix
+            const int e0 = q * 4 - s.head;
+            jv = make_int4(0, 0, 0, 0);
+            xv = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (e0 + 0 < s.len) { jv.x = __ldg(a.indices + off + 0); xv.x = a.data[off + 0]; }
+            if (e0 + 1 < s.len) { jv.y = __ldg(a.indices + off + 1); xv.y = a.data[off + 1]; }
+            if (e0 + 2 < s.len) { jv.z = __ldg(a.indices + off + 2); xv.z = a.data[off + 2]; }
+          }
         }
       };
-      auto compute_step = [&](const Seg& s, int q0, const int4& jv, const float4& xv) {
-        const int q = q0 + lane;
+      auto compute_step = [&](const Seg& s, int st, const int4& jv, const float4& xv) {
+        const int q = st * 32 + lane;
         const int e0 = q * 4 - s.head;
-        const bool full = e0 >= 0 && e0 + 4 <= s.len;
-        float* dq = a.data + s.abeg + 4LL * q;
-        if (__all_sync(0xffffffffu, full)) {
+        float* dq = a.data + (s.abeg + 4 * q);
+        if (interior(s, st)) {
           *reinterpret_cast<float4*>(dq) = quad(std::false_type{}, jv, xv, s.scale, e0, s.len);
         } else if (q < s.nq) {
           const float4 r = quad(std::true_type{}, jv, xv, s.scale, e0, s.len);
-          if (full) {
+          if (e0 >= 0 && e0 + 4 <= s.len) {
             *reinterpret_cast<float4*>(dq) = r;
           } else {
             if ((unsigned)(e0 + 0) < (unsigned)s.len) dq[0] = r.x;
@@ -454,33 +514,39 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
         }
       };
       {
-        int ri = 0;
-        Seg S = seg_of(0);
-        while (S.nq == 0 && ++ri < kFuRowsPerGrab) S = seg_of(ri);
-        if (ri < kFuRowsPerGrab) {
-          int q0 = 0;
-          int4 jc = make_int4(0, 0, 0, 0);
-          float4 xc = make_float4(0.f, 0.f, 0.f, 0.f);
-          load_step(S, q0, jc, xc);
-          for (;;) {
-            Seg N = S;
-            int nq0 = q0 + 32, nri = ri;
-            if (nq0 >= S.nq) {
-              nq0 = 0;
+        Seg S;
+        S.nq = 0;
+        int ri = -1;
+        while (++ri < kFuRowsPerGrab) { S = seg_of(ri); if (S.nq) break; }
+        int4 jn = make_int4(0, 0, 0, 0);
+        float4 xn4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (ri < kFuRowsPerGrab) load_step(S, 0, jn, xn4);
+        while (ri < kFuRowsPerGrab) {
+          const int nsteps = (S.nq + 31) >> 5;
+          int nri = ri;
+          // the next row's segment (of this grab or the first of the next) goes to L2 now
+          if (ri + 1 < kFuRowsPerGrab) l2_prefetch(mbeg, mend, ri + 1);
+          else if (next_ok) l2_prefetch(nbeg, nend, 0);
+#pragma unroll 1
+          for (int st = 0; st < nsteps; ++st) {
+            const int4 jc = jn;
+            const float4 xc = xn4;
+            if (st + 1 < nsteps) {
+              load_step(S, st + 1, jn, xn4);
+            } else {                                      // prefetch the next segment's first step
+              Seg N;
               N.nq = 0;
               while (++nri < kFuRowsPerGrab) { N = seg_of(nri); if (N.nq) break; }
+              if (nri < kFuRowsPerGrab) load_step(N, 0, jn, xn4);
             }
-            const bool has_next = nri < kFuRowsPerGrab;
-            int4 jn = make_int4(0, 0, 0, 0);
-            float4 xn4 = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (has_next) load_step(N, nq0, jn, xn4);
-            compute_step(S, q0, jc, xc);
-            if (!has_next) break;
-            S = N; q0 = nq0; ri = nri; jc = jn; xc = xn4;
+            compute_step(S, st, jc, xc);
           }
+          ri = nri;
+          if (ri < kFuRowsPerGrab) S = seg_of(ri);
         }
       }
-      r0 = __shfl_sync(0xffffffffu, pending, 0);
+      r0 = rnext; mbeg = nbeg; mend = nend; mscale = nscale;
+      rnext = __shfl_sync(0xffffffffu, pending, 0);
     }
     done = __syncthreads_or(saw_end);
     // flush this CTA's accumulators into the global double sums and clear them

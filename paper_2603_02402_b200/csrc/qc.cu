@@ -14,6 +14,8 @@
 //   * optionally the row split table consumed by the fused pass (fused.cu): for every row,
 //     the number of entries with column < k * RSC_SPLIT_WIDTH, found by comparing the column
 //     block of a lane's last entry with its neighbour's (rows must be sorted).
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace rsc {
@@ -21,7 +23,7 @@ namespace rsc {
 constexpr int kQcThreads = 1024;
 constexpr int kQcWarps = kQcThreads / 32;
 constexpr int kQcRowsPerGrab = 4;
-constexpr int kQcUnroll = 2;                 // 2 x 128 entries per warp iteration
+constexpr int kQcAhead = 6;                  // L2 look-ahead of a warp, in steps of 128 entries
 constexpr uint32_t kQcMaxFast = 511u;        // largest count that takes the shared-memory path
 constexpr int kQcMaxRowBudget = 2047 - kQcRowsPerGrab;   // rows per flush period incl. the last grab
 
@@ -52,33 +54,28 @@ __device__ __forceinline__ long long warp_sum_ll(long long v) {
   return v;
 }
 
-// shared-memory atomic add on a 32-bit shared address, executed only when `on` is set
-// (a predicated ATOMS instead of a branch); returns the previous word (0 when skipped)
-__device__ __forceinline__ uint32_t atoms_add_if(uint32_t saddr, uint32_t v, bool on) {
-  uint32_t old = 0u;
-  asm volatile(
-      "{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %3, 0;\n\t@p atom.shared.add.u32 %0, [%1], %2;\n\t}"
-      : "+r"(old)
-      : "r"(saddr), "r"(v), "r"((uint32_t)on)
-      : "memory");
+// native shared atomic add on a 32-bit shared address, returning the previous word
+__device__ __forceinline__ uint32_t qc_atoms_add(uint32_t saddr, uint32_t v) {
+  uint32_t old;
+  asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(saddr), "r"(v));
   return old;
 }
 
 template <bool SPLITS>
 __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a) {
-  extern __shared__ __align__(16) uint32_t qsm[];      // [G] packed flag | count | total
+  extern __shared__ __align__(16) uint32_t qsm[];      // [G] packed flag | count | total, + 1 spare
   const int G = a.n_cols;
   const int tid = threadIdx.x, lane = tid & 31;
   const int K = a.n_fine;
-  const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(qsm);
+  uint32_t sbase = (uint32_t)__cvta_generic_to_shared(qsm);
+  asm volatile("mov.u32 %0, %0;" : "+r"(sbase));       // keep it in a register
   __shared__ unsigned s_rows;
 
-  for (int g = tid; g < G; g += kQcThreads)
-    qsm[g] = (a.flags != nullptr && a.flags[g] != 0) ? 0x80000000u : 0u;
+  for (int g = tid; g <= G; g += kQcThreads)
+    qsm[g] = (g < G && a.flags != nullptr && a.flags[g] != 0) ? 0x80000000u : 0u;
 
   // -1: the CTA's row budget is used up (flush first); >= n_rows: the matrix is exhausted
-  // (only lane 0 holds the result; it is broadcast when needed, so the L2 round trip of the
-  // atomic overlaps the rows being processed)
+  // (only lane 0 holds the result; it is broadcast when needed)
   auto grab_issue = [&]() -> long long {
     long long r = -1;
     if (lane == 0) {
@@ -88,117 +85,161 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
     }
     return r;
   };
+  auto load_ptrs = [&](long long r0) -> int64_t {       // lanes 0..RG: indptr[r0 + lane]
+    int64_t p = 0;
+    if (lane <= kQcRowsPerGrab && r0 + lane <= a.n_rows) p = a.indptr[r0 + lane];
+    return p;
+  };
+  // L2 prefetch of elements [p0, p0 + count) of both arrays (p0 a multiple of 4), issued by
+  // one lane: bounded look-ahead, so nothing is evicted before it is used
+  auto l2_prefetch = [&](int64_t p0, int count) {
+    const int64_t room = a.nnz - p0;
+    if (room < count) count = (int)(room > 0 ? room : 0) & ~3;
+    if (lane == 0 && count > 0) {
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a.indices + p0), "r"(count * 4));
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a.data + p0), "r"(count * 4));
+    }
+  };
+  // per-lane partial sums of the current row
+  unsigned t32, m32, n32;                               // fast path (counts <= 511)
+  long long T64, M64;                                   // slow path (large / negative counts)
+
+  // One quad of 4 consecutive entries.  EDGE: only entries e0 + k in [0, len) belong to the
+  // row; the others add 0 to the spare word qsm[G].
+  auto quad = [&](auto edge_tag, const int4 jv, const float4 xv, int e0, int len) {
+    constexpr bool EDGE = decltype(edge_tag)::value;
+    const int j[4] = {jv.x, jv.y, jv.z, jv.w};
+    const float x[4] = {xv.x, xv.y, xv.z, xv.w};
+    int xi[4];
+    bool valid[4];
+    bool slow = false;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      valid[k] = !EDGE || (unsigned)(e0 + k) < (unsigned)len;
+      xi[k] = __float2int_rz(x[k]);
+      slow = slow || (valid[k] && (unsigned)xi[k] > kQcMaxFast);
+    }
+    if (!slow) {
+      uint32_t old[4], xf[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const bool nz = valid[k] && x[k] != 0.0f;
+        xf[k] = valid[k] ? (uint32_t)xi[k] : 0u;
+        const uint32_t jj = valid[k] ? (uint32_t)j[k] : (uint32_t)G;
+        old[k] = qc_atoms_add(sbase + (jj << 2), xf[k] + (nz ? 0x100000u : 0u));
+        n32 += nz ? 1u : 0u;
+        t32 += xf[k];
+      }
+#pragma unroll
+      for (int k = 0; k < 4; ++k) m32 += xf[k] & (uint32_t)((int)old[k] >> 31);
+    } else {                                            // rare: counts > 511, negative, non-finite
+#pragma unroll 1
+      for (int k = 0; k < 4; ++k) {
+        if (!valid[k]) continue;
+        const float xv1 = k == 0 ? x[0] : k == 1 ? x[1] : k == 2 ? x[2] : x[3];
+        const int jj = k == 0 ? j[0] : k == 1 ? j[1] : k == 2 ? j[2] : j[3];
+        const int xi1 = __float2int_rz(xv1);
+        if ((unsigned)xi1 <= kQcMaxFast) {
+          const bool nz = xv1 != 0.0f;
+          const uint32_t o = qc_atoms_add(sbase + ((uint32_t)jj << 2), (uint32_t)xi1 + (nz ? 0x100000u : 0u));
+          n32 += nz ? 1u : 0u;
+          t32 += (uint32_t)xi1;
+          m32 += (uint32_t)xi1 & (uint32_t)((int)o >> 31);
+        } else {
+          const long long xl = (long long)xv1;
+          n32 += xv1 != 0.0f ? 1u : 0u;
+          T64 += xl;
+          if (qsm[jj] >> 31) M64 += xl;
+          if (a.gene_n_cells != nullptr && xv1 != 0.0f) atomicAdd(&a.gene_n_cells[jj], 1);
+          if (xl != 0 && a.gene_total != nullptr)
+            atomicAdd(&a.gene_total[jj], (unsigned long long)xl);
+        }
+      }
+    }
+  };
 
   int done;
   do {
     if (tid == 0) s_rows = 0u;
     __syncthreads();
     int saw_end = 0;
+    // Grabs are pipelined two deep (see fused.cu): row range of grab g + 1 known and its
+    // indptr entries loaded while grab g is processed; every row is prefetched into L2 one
+    // row ahead of its use.
     long long r0 = __shfl_sync(0xffffffffu, grab_issue(), 0);
+    int64_t mptr = (r0 >= 0 && r0 < a.n_rows) ? load_ptrs(r0) : 0;
+    long long rnext = __shfl_sync(0xffffffffu, grab_issue(), 0);
     while (r0 >= 0) {
       if (r0 >= a.n_rows) { saw_end = 1; break; }
       const long long pending = grab_issue();
-      // lanes 0..RG fetch the row bounds of this grab
-      int64_t mptr = 0;
-      if (lane <= kQcRowsPerGrab && r0 + lane <= a.n_rows) mptr = a.indptr[r0 + lane];
+      const bool next_ok = rnext >= 0 && rnext < a.n_rows;
+      const int64_t nptr = next_ok ? load_ptrs(rnext) : 0;
       const int nr = (int)min((long long)kQcRowsPerGrab, a.n_rows - r0);
+      const int64_t gend = __shfl_sync(0xffffffffu, mptr, nr);   // end of the grab's contiguous range
 #pragma unroll 1
       for (int ri = 0; ri < nr; ++ri) {
         const long long row = r0 + ri;
         const int64_t beg = __shfl_sync(0xffffffffu, mptr, ri);
         const int64_t end = __shfl_sync(0xffffffffu, mptr, ri + 1);
-        // all positions below are 32-bit offsets from the 4-aligned start of the row
+        if (ri == 1 && next_ok)                         // the head of the next grab
+          l2_prefetch(__shfl_sync(0xffffffffu, nptr, 0) & ~3LL, kQcAhead * 128);
+        // quads at 16-byte aligned offsets; e = index relative to the row start
         const int64_t abeg = beg & ~3LL;
-        const int head = (int)(beg - abeg);             // entries of the previous row in the first quad
+        const int head = (int)(beg - abeg);
         const int len = (int)(end - beg);
-        const int span = head + len;
-        const int64_t room = a.nnz - abeg;              // a quad at offset r is a vector load iff r + 4 <= vlim
-        const int vlim = room > 0x7fffffffLL ? 0x7fffffff : (int)room;
-        const int32_t* ip = a.indices + abeg + lane * 4;
-        const float* dp = a.data + abeg + lane * 4;
-        unsigned t32 = 0, m32 = 0, n32 = 0;             // fast-path partial sums of this lane
-        long long T64 = 0, M64 = 0;                     // slow-path (large / negative counts)
-        int carry_f = -1;                               // column block of the previous entry
+        const int nq = len > 0 ? (head + len + 3) >> 2 : 0;
+        const int nsteps = (nq + 31) >> 5;
+        t32 = 0; m32 = 0; n32 = 0; T64 = 0; M64 = 0;
         uint32_t* sp = SPLITS ? a.splits + (size_t)row * (size_t)(K + 1) : nullptr;
-        for (int rb = 0; rb < span; rb += 128 * kQcUnroll, ip += 128 * kQcUnroll, dp += 128 * kQcUnroll) {
-          int j[kQcUnroll][4];
-          float x[kQcUnroll][4];
-#pragma unroll
-          for (int u = 0; u < kQcUnroll; ++u) {
-            const int r = rb + u * 128 + lane * 4;
-            if (r + 4 <= vlim && r < span) {
-              const int4 jv = __ldg(reinterpret_cast<const int4*>(ip + u * 128));
-              const float4 xv = __ldg(reinterpret_cast<const float4*>(dp + u * 128));
-              j[u][0] = jv.x; j[u][1] = jv.y; j[u][2] = jv.z; j[u][3] = jv.w;
-              x[u][0] = xv.x; x[u][1] = xv.y; x[u][2] = xv.z; x[u][3] = xv.w;
-            } else {
-#pragma unroll
-              for (int k = 0; k < 4; ++k) {             // last quad of the matrix, or past the row
-                const bool ok = r + k < span && r + k < vlim;
-                j[u][k] = ok ? __ldg(ip + u * 128 + k) : 0;
-                x[u][k] = ok ? __ldg(dp + u * 128 + k) : 0.0f;
-              }
-            }
+        auto interior = [&](int st) -> bool {
+          return (st > 0 || head == 0) && (st * 128 + 128 <= head + len);
+        };
+        auto load_step = [&](int st, int4& jv, float4& xv) {
+          const int q = st * 32 + lane;
+          const int64_t off = abeg + 4 * q;
+          if (interior(st) || (q < nq && off + 4 <= a.nnz)) {
+            jv = __ldg(reinterpret_cast<const int4*>(a.indices + off));
+            xv = __ldg(reinterpret_cast<const float4*>(a.data + off));
+          } else if (q < nq) {                          // the last quad of the whole matrix
+            const int e0 = q * 4 - head;
+            jv = make_int4(0, 0, 0, 0);
+            xv = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (e0 + 0 < len) { jv.x = __ldg(a.indices + off + 0); xv.x = __ldg(a.data + off + 0); }
+            if (e0 + 1 < len) { jv.y = __ldg(a.indices + off + 1); xv.y = __ldg(a.data + off + 1); }
+            if (e0 + 2 < len) { jv.z = __ldg(a.indices + off + 2); xv.z = __ldg(a.data + off + 2); }
           }
-#pragma unroll
-          for (int u = 0; u < kQcUnroll; ++u) {
-            const int e0 = rb + u * 128 + lane * 4 - head;   // row-relative index of the quad's first entry
-            if (SPLITS) {
-              // column block of every entry: -1 before the row, K after it
-              int f[4];
-#pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                const int e = e0 + k;
-                f[k] = e < 0 ? -1 : (e < len ? (j[u][k] >> RSC_SPLIT_SHIFT) : K);
-              }
-              int fp = __shfl_up_sync(0xffffffffu, f[3], 1);
-              if (lane == 0) fp = carry_f;
-              carry_f = __shfl_sync(0xffffffffu, f[3], 31);
-#pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                if (f[k] != fp) {                       // first entry of block f[k] (and of skipped ones)
-                  const uint32_t pos = (uint32_t)min(e0 + k, len);
+        };
+        int4 jn = make_int4(0, 0, 0, 0);
+        float4 xn = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (nsteps > 0) load_step(0, jn, xn);
 #pragma unroll 1
-                  for (int kk = fp + 1; kk <= f[k]; ++kk) sp[kk] = pos;
-                }
-                fp = f[k];
-              }
-            }
-            bool any_slow = false;
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-              const bool valid = (unsigned)(e0 + k) < (unsigned)len;
-              const float xv = x[u][k];
-              const int xi = __float2int_rz(xv);
-              const bool nz = valid && xv != 0.0f;
-              const bool fast = valid && (unsigned)xi <= kQcMaxFast;
-              any_slow |= valid && !fast;
-              const unsigned xf = fast ? (unsigned)xi : 0u;
-              const uint32_t old =
-                  atoms_add_if(sbase + ((uint32_t)j[u][k] << 2), xf + (nz ? 0x100000u : 0u), fast);
-              n32 += nz ? 1u : 0u;
-              t32 += xf;
-              m32 += xf & (uint32_t)((int)old >> 31);
-            }
-            if (any_slow) {                             // rare: counts > 511, negative or non-finite values
-#pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                const bool valid = (unsigned)(e0 + k) < (unsigned)len;
-                const float xv = x[u][k];
-                if (!valid || (unsigned)__float2int_rz(xv) <= kQcMaxFast) continue;
-                const int jj = j[u][k];
-                const long long xl = (long long)xv;
-                T64 += xl;
-                if (qsm[jj] >> 31) M64 += xl;
-                if (a.gene_n_cells != nullptr) atomicAdd(&a.gene_n_cells[jj], 1);
-                if (xl != 0 && a.gene_total != nullptr)
-                  atomicAdd(&a.gene_total[jj], (unsigned long long)xl);
-              }
-            }
+        for (int st = 0; st < nsteps; ++st) {
+          const int4 jc = jn;
+          const float4 xc = xn;
+          if (st + 1 < nsteps) load_step(st + 1, jn, xn);
+          {
+            const int64_t pf = abeg + (int64_t)(st + kQcAhead) * 128;
+            if (pf < gend) l2_prefetch(pf, 128);
           }
+          const int q = st * 32 + lane;
+          const int e0 = q * 4 - head;
+          const bool inter = interior(st);
+          if (inter) quad(std::false_type{}, jc, xc, e0, len);
+          else if (q < nq) quad(std::true_type{}, jc, xc, e0, len);
         }
         if (SPLITS) {
-          for (int k = carry_f + 1 + lane; k <= K; k += 32) sp[k] = (uint32_t)len;
+          // split table of the row: lane k finds #{entries with column < k * RSC_SPLIT_WIDTH} by
+          // binary search in the (sorted) row, whose lines were just streamed (L2 / L1 hits)
+          for (int k = lane; k <= K; k += 32) {
+            const int32_t bound = k << RSC_SPLIT_SHIFT;
+            int lo = 0, hi = len;
+            if (k == 0) hi = 0;
+            while (lo < hi) {
+              const int mid = (lo + hi) >> 1;
+              if (__ldg(a.indices + beg + mid) < bound) lo = mid + 1; else hi = mid;
+            }
+            sp[k] = (uint32_t)lo;
+          }
         }
         long long T, M;
         if (__any_sync(0xffffffffu, (T64 | M64) != 0)) {
@@ -217,7 +258,8 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
           if (a.cell_flag_pct) a.cell_flag_pct[row] = (float)(100.0 * (double)M / (double)T);
         }
       }
-      r0 = __shfl_sync(0xffffffffu, pending, 0);
+      r0 = rnext; mptr = nptr;
+      rnext = __shfl_sync(0xffffffffu, pending, 0);
     }
     done = __syncthreads_or(saw_end);
     // flush and clear the CTA's table (the flag bit stays)
@@ -300,7 +342,7 @@ int launch_qc(const rsc_csr& X, const uint8_t* gene_flags, int64_t* cell_total_i
   a.n_rows = X.n_rows;
   a.nnz = X.nnz;
   a.n_cols = X.n_cols;
-  const size_t smem = sizeof(uint32_t) * (size_t)X.n_cols + 16;
+  const size_t smem = sizeof(uint32_t) * ((size_t)X.n_cols + 1) + 16;   // + the spare word
   a.n_fine = split_blocks(X.n_cols);
   a.indptr = X.indptr; a.indices = X.indices; a.data = X.data; a.flags = gene_flags;
   a.cell_total = cell_total_i64; a.cell_total_f32 = cell_total_f32; a.cell_n_genes = cell_n_genes;
