@@ -90,16 +90,16 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
     if (lane <= kQcRowsPerGrab && r0 + lane <= a.n_rows) p = a.indptr[r0 + lane];
     return p;
   };
-  // L2 prefetch of elements [p0, p0 + count) of both arrays (p0 a multiple of 4), issued by
-  // one lane: bounded look-ahead, so nothing is evicted before it is used
-  auto l2_prefetch = [&](int64_t p0, int count) {
-    const int64_t room = a.nnz - p0;
-    if (room < count) count = (int)(room > 0 ? room : 0) & ~3;
-    if (lane == 0 && count > 0) {
-      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a.indices + p0), "r"(count * 4));
-      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a.data + p0), "r"(count * 4));
+  // L2 prefetch of the 128 entries at p0 (both arrays): lanes 0..3 touch one 128-byte line each;
+  // bounded look-ahead, so nothing is evicted before it is used
+  auto l2_prefetch = [&](int64_t p0) {
+    const int64_t p = p0 + lane * 32;
+    if (lane < 4 && p < a.nnz) {
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(a.indices + p));
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(a.data + p));
     }
   };
+  auto opaque = [](int v) -> int { asm volatile("mov.u32 %0, %0;" : "+r"(v)); return v; };
   // per-lane partial sums of the current row
   unsigned t32, m32, n32;                               // fast path (counts <= 511)
   long long T64, M64;                                   // slow path (large / negative counts)
@@ -182,50 +182,48 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
         const int64_t beg = __shfl_sync(0xffffffffu, mptr, ri);
         const int64_t end = __shfl_sync(0xffffffffu, mptr, ri + 1);
         if (ri == 1 && next_ok)                         // the head of the next grab
-          l2_prefetch(__shfl_sync(0xffffffffu, nptr, 0) & ~3LL, kQcAhead * 128);
-        // quads at 16-byte aligned offsets; e = index relative to the row start
+          for (int i = 0; i < kQcAhead; ++i) l2_prefetch((__shfl_sync(0xffffffffu, nptr, 0) & ~3LL) + i * 128);
+        // quads at 16-byte aligned offsets; e = index relative to the row start.  The lane's
+        // pointers / e0 advance by 128 entries per step (no per-step address arithmetic).
         const int64_t abeg = beg & ~3LL;
         const int head = (int)(beg - abeg);
         const int len = (int)(end - beg);
-        const int nq = len > 0 ? (head + len + 3) >> 2 : 0;
-        const int nsteps = (nq + 31) >> 5;
+        const int span = opaque(len > 0 ? head + len : 0);
         t32 = 0; m32 = 0; n32 = 0; T64 = 0; M64 = 0;
         uint32_t* sp = SPLITS ? a.splits + (size_t)row * (size_t)(K + 1) : nullptr;
-        auto interior = [&](int st) -> bool {
-          return (st > 0 || head == 0) && (st * 128 + 128 <= head + len);
-        };
-        auto load_step = [&](int st, int4& jv, float4& xv) {
-          const int q = st * 32 + lane;
-          const int64_t off = abeg + 4 * q;
-          if (interior(st) || (q < nq && off + 4 <= a.nnz)) {
-            jv = __ldg(reinterpret_cast<const int4*>(a.indices + off));
-            xv = __ldg(reinterpret_cast<const float4*>(a.data + off));
-          } else if (q < nq) {                          // the last quad of the whole matrix
-            const int e0 = q * 4 - head;
+        const int32_t* ip = a.indices + abeg + lane * 4;
+        const float* dp = a.data + abeg + lane * 4;
+        int e0 = lane * 4 - head;
+        // every quad of the row lies inside the arrays (false only for the matrix's last row)
+        const bool vec_ok = opaque(abeg + ((span + 3) & ~3) <= a.nnz ? 1 : 0) != 0;
+        auto load_q = [&](const int32_t* ipq, const float* dpq, int e, int4& jv, float4& xv) {
+          if (e >= len) return;                         // quad past the row
+          if (vec_ok) {
+            jv = __ldg(reinterpret_cast<const int4*>(ipq));
+            xv = __ldg(reinterpret_cast<const float4*>(dpq));
+          } else {
             jv = make_int4(0, 0, 0, 0);
             xv = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (e0 + 0 < len) { jv.x = __ldg(a.indices + off + 0); xv.x = __ldg(a.data + off + 0); }
-            if (e0 + 1 < len) { jv.y = __ldg(a.indices + off + 1); xv.y = __ldg(a.data + off + 1); }
-            if (e0 + 2 < len) { jv.z = __ldg(a.indices + off + 2); xv.z = __ldg(a.data + off + 2); }
+            if (e + 0 < len) { jv.x = __ldg(ipq + 0); xv.x = __ldg(dpq + 0); }
+            if (e + 1 < len) { jv.y = __ldg(ipq + 1); xv.y = __ldg(dpq + 1); }
+            if (e + 2 < len) { jv.z = __ldg(ipq + 2); xv.z = __ldg(dpq + 2); }
+            if (e + 3 < len) { jv.w = __ldg(ipq + 3); xv.w = __ldg(dpq + 3); }
           }
         };
         int4 jn = make_int4(0, 0, 0, 0);
         float4 xn = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (nsteps > 0) load_step(0, jn, xn);
-#pragma unroll 1
-        for (int st = 0; st < nsteps; ++st) {
+        if (span > 0) load_q(ip, dp, e0, jn, xn);
+        int64_t pf = abeg + kQcAhead * 128;             // L2 look-ahead position (lane-uniform)
+#pragma unroll 2
+        for (int base = 0; base < span; base += 128) {
           const int4 jc = jn;
           const float4 xc = xn;
-          if (st + 1 < nsteps) load_step(st + 1, jn, xn);
-          {
-            const int64_t pf = abeg + (int64_t)(st + kQcAhead) * 128;
-            if (pf < gend) l2_prefetch(pf, 128);
-          }
-          const int q = st * 32 + lane;
-          const int e0 = q * 4 - head;
-          const bool inter = interior(st);
+          load_q(ip + 128, dp + 128, e0 + 128, jn, xn);
+          if (pf < gend) l2_prefetch(pf);
+          const bool inter = (base > 0 || head == 0) && (base + 128 <= span);
           if (inter) quad(std::false_type{}, jc, xc, e0, len);
-          else if (q < nq) quad(std::true_type{}, jc, xc, e0, len);
+          else if (e0 < len) quad(std::true_type{}, jc, xc, e0, len);
+          ip += 128; dp += 128; e0 += 128; pf += 128;
         }
         if (SPLITS) {
           // split table of the row: lane k finds #{entries with column < k * RSC_SPLIT_WIDTH} by
