@@ -38,7 +38,11 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number (1-5)")
     ap.add_argument("--cells", type=int, default=None, help="override the row count (debug)")
-    ap.add_argument("--which-moments", type=int, default=3, help="1 log, 2 linear, 3 both")
+    ap.add_argument("--which-moments", type=int, default=1,
+                    help="moment sets of the fused pass: 1 log scale (north_star's chain, default), "
+                         "2 linear scale (scanpy's Seurat input), 3 both")
+    ap.add_argument("--no-variants", action="store_true",
+                    help="skip the extra timing of the other which-moments settings")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -225,6 +229,26 @@ def main():
         total_ms_max, nnz_all = total_ms, float(nnz)
     value = nnz_all * args.steps / (total_ms_max / 1e3)
 
+    # ---- the other moment-set settings of the fused pass, timed the same way (N=1 only)
+    variants = None
+    if not args.no_variants and world == 1:
+        variants = {}
+        for wm in (1, 2, 3):
+            if wm == args.which_moments:
+                continue
+            vp = Preprocessor(X.n_rows, X.n_cols, nnz, cfg.target_sum, cfg.n_top, cfg.n_bins, 1,
+                              wm, bool(wm & 2), device=dev)
+            vevs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(8)]
+            for k in range(8):
+                data.copy_(pristine)
+                vp.run_staged(X, flags, vevs[k] if k >= 3 else None)
+            torch.cuda.synchronize()
+            tf = [e[1].elapsed_time(e[2]) for e in vevs[3:]]
+            tc = [e[0].elapsed_time(e[3]) for e in vevs[3:]]
+            variants[f"which_moments={wm}"] = {"fused_ms": sum(tf) / len(tf), "chain_ms": sum(tc) / len(tc),
+                                               "chain_nnz_per_s": nnz / (sum(tc) / len(tc) / 1e3)}
+            del vp
+
     # ---- end to end through the host entry point (rank-local; N=1 only)
     e2e = None
     if not args.no_e2e and world == 1:
@@ -286,10 +310,11 @@ def main():
                    "n_cells_per_gpu": X.n_rows, "n_genes": X.n_cols, "nnz_per_gpu": nnz,
                    "target_sum": cfg.target_sum, "n_top": cfg.n_top, "n_bins": cfg.n_bins,
                    "which_moments": args.which_moments,
+                   "moments": {1: "log scale (of x'')", 2: "linear scale (of x')", 3: "log + linear"}[args.which_moments & 3],
                    "l2": "inputs (>= 8 B/nnz) larger than L2; data restored from a pristine copy "
                          "between steps (untimed)",
                    "parallelism": "1 GPU" if world == 1 else f"row-sharded x{world} + all-reduce of per-gene sums"},
-        "roofline": roofline, "stages": stages, "cpu_baseline": cpu, "e2e": e2e,
+        "roofline": roofline, "stages": stages, "variants": variants, "cpu_baseline": cpu, "e2e": e2e,
         "gpu_launches": int(launches), "clocks": sampler.summary(),
     }
     print(json.dumps(line))

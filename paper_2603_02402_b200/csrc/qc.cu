@@ -23,7 +23,10 @@ namespace rsc {
 constexpr int kQcThreads = 1024;
 constexpr int kQcWarps = kQcThreads / 32;
 constexpr int kQcRowsPerGrab = 4;
-constexpr int kQcAhead = 6;                  // L2 look-ahead of a warp, in steps of 128 entries
+#ifndef RSC_QC_AHEAD
+#define RSC_QC_AHEAD 4
+#endif
+constexpr int kQcAhead = RSC_QC_AHEAD;                  // L2 look-ahead of a warp, in steps of 128 entries
 constexpr uint32_t kQcMaxFast = 511u;        // largest count that takes the shared-memory path
 constexpr int kQcMaxRowBudget = 2047 - kQcRowsPerGrab;   // rows per flush period incl. the last grab
 

@@ -334,8 +334,9 @@ def test_fused_equals_unfused_bitwise_and_is_order_independent():
 
 
 def test_fixed_point_extreme_ranges():
-    """Rows whose totals differ by 2^20 (x' from ~1e-2 to target_sum) and both target sums: the
-    fixed-point windows keep every addend's 31 significant bits."""
+    """Rows whose totals differ by 2^26 (x' from ~1e-4 to target_sum) and both target sums: the
+    integer accumulators are exact inside their window (one-word and two-word addends), and the
+    values below it (the deep cell's) take the global double path."""
     from paper_2603_02402_b200 import binding as B
     rng = np.random.default_rng(7)
     n, G = 64, 3000
@@ -347,6 +348,7 @@ def test_fixed_point_extreme_ranges():
     dense[0, :] = 0; dense[0, 5] = 7                      # one gene takes the whole cell: x' = s
     dense[1, :2000] = 500.0                               # T = 1e6: x' = s / 2000 * ... tiny
     dense[2, 5] = 1.0; dense[2, 100:1100] = 1000.0        # x' of gene 5 ~ s * 1e-6
+    dense[3, :] = 0; dense[3, 10:74] = 1.0e6; dense[3, 5] = 3.0   # T = 6.4e7: x' below any window
     indptr = np.zeros(n + 1, dtype=np.int64)
     r, c = np.nonzero(dense)
     np.cumsum(np.bincount(r, minlength=n), out=indptr[1:])
