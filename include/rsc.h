@@ -79,7 +79,7 @@ const char* rsc_version(void);
 uint64_t rsc_kernel_launch_count(void);
 /* Process-wide tuning / testing knobs (not needed in normal use; defaults in brackets):
  *   "fused_row_budget" [4000]  rows a CTA of the fused pass takes between two flushes of its
- *                              fixed-point accumulators (1..4092; 4096 rows cannot overflow)
+ *                              integer accumulators (1..4092; 4096 rows cannot overflow)
  *   "qc_row_budget"    [2043]  the same for the QC pass's 11-bit count fields (1..2043)
  *   "grid_ctas"        [0]     CTAs of the streaming kernels, 0 = one per SM
  *   "force_generic"    [0]     1 = always take the generic L2-atomic kernels
@@ -151,10 +151,14 @@ int rsc_gene_moments(const rsc_csr* X, int transform, int ddof,
  * accumulated in double precision.
  *   which_moments: bit0 RSC_MOMENTS_LOG -> mean_log/var_log, bit1 RSC_MOMENTS_LIN ->
  *   mean_lin/var_lin (the matching pointers are then required).  By default the sums are
- *   accumulated on chip in 64-bit fixed point (order-independent; every addend keeps >= 31
- *   significant bits for non-negative data with x' >= target_sum * 2^-30, see DESIGN.md
- *   section 5); bit2 RSC_MOMENTS_FP64_ACC selects double-precision accumulators instead
- *   (any value range, slower).  Data must be non-negative for the fixed-point path.
+ *   accumulated on chip as EXACT integers (every value v is scaled by a power of two chosen on
+ *   the device from the largest cell total, so that v * 2^k is an integer; S1 in 64 bits, S2
+ *   in 96 bits, order-independent); values more than 2^19 times smaller
+ *   than target_sum's binade, negative values and NaNs are added to the global double sums
+ *   directly (same result, slower).  bit2 RSC_MOMENTS_FP64_ACC selects double-precision
+ *   shared-memory accumulators instead (any value range, slower).
+ *   X->indices and X->data must be 16-byte aligned for the streaming kernel (else the generic
+ *   kernel serves the call: same results).
  *   row_splits: optional row split table of X (from rsc_qc_metrics / rsc_row_splits);
  *   NULL -> computed into the workspace when needed.
  *   cell_total_i64 is required (from rsc_qc_metrics).
