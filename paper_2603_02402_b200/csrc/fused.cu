@@ -46,6 +46,7 @@ constexpr int kFuThreads = RSC_FU_THREADS;
 constexpr int kFuRowsPerGrab = 4;
 constexpr int kMaxGroups = 64;
 constexpr int kSetWords = 5;               // u32 words per gene and moment set (w0 w1 s0 s1 s2)
+constexpr double kRowCost = 200.0;         // per-row-segment overhead, in entries (plan kernel)
 constexpr int kMaxRangeBits = 19;          // 2^k * v_max <= 2^(23 + 19) = 2^42
 
 struct MomentScale {                       // one per moment set; written by fused_plan_kernel
@@ -123,15 +124,15 @@ __device__ inline MomentScale make_scale(double v_min, double v_max) {
 // ------------------------------------------------------------------ plan (1 CTA)
 __global__ void __launch_bounds__(1024)
 fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid, float target_sum,
-                  const int32_t* __restrict__ gene_n_cells) {
+                  long long n_rows, const int32_t* __restrict__ gene_n_cells) {
   __shared__ double mass[kMaxGroups];
   const int tid = threadIdx.x;
   const int ng = (K + fine_per_group - 1) / fine_per_group;
   if (tid < kMaxGroups) mass[tid] = 0.0;
   __syncthreads();
-  const int gw = fine_per_group << RSC_SPLIT_SHIFT;       // genes per group
-  for (int c = 0; c < ng; ++c) {
-    const int g0 = c * gw, g1 = min(G, g0 + gw);
+  for (int c = 0; c < ng; ++c) {                          // group c = blocks [c K / ng, (c + 1) K / ng)
+    const int g0 = ((c * K) / ng) << RSC_SPLIT_SHIFT;
+    const int g1 = min(G, (((c + 1) * K) / ng) << RSC_SPLIT_SHIFT);
     double m = 0.0;
     for (int g = g0 + tid; g < g1; g += 1024) {
       const int v = gene_n_cells ? gene_n_cells[g] : 1;
@@ -142,8 +143,11 @@ fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid, f
   }
   __syncthreads();
   if (tid == 0) {
+    // cost of a group = its entries + a per-row overhead (every CTA of the group walks a
+    // segment of EVERY row: grab, metadata, edge steps ~ the work of kRowCost entries), so a
+    // group of few, sparse columns still gets the CTAs its row count needs
     double total = 0.0;
-    for (int c = 0; c < ng; ++c) total += mass[c];
+    for (int c = 0; c < ng; ++c) { mass[c] += (double)n_rows * kRowCost; total += mass[c]; }
     int n[kMaxGroups];
     int sum = 0;
     for (int c = 0; c < ng; ++c) {
@@ -285,6 +289,42 @@ __device__ __forceinline__ void acc_quad(uint32_t base, const uint32_t (&so)[4],
   for (int k = 0; k < 4; ++k) reds_inc_if(sa[k] + 16, carry_of(o[k], q1[k]) != 0u);
 }
 
+// 2^23 <= t < 2^42: an exact integer of at most two words
+__device__ __forceinline__ bool in_window_wide(float t) {
+  return (__float_as_uint(t) - 0x4B000000u) < 0x09800000u;       // 2^42 = 0x54800000
+}
+
+// acc_quad for two-word a (a < 2^42, so a * a < 2^84): S1 in (w0, w1), S2 in (s0, s1, s2)
+__device__ __forceinline__ void acc_quad_wide(uint32_t base, const uint32_t (&so)[4],
+                                              const unsigned long long (&a)[4]) {
+  uint32_t sa[4], o[4], o0[4], q0[4], q1[4], q2[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { sa[k] = base + so[k]; o[k] = atoms_add(sa[k], (uint32_t)a[k]); }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const unsigned long long plo = a[k] * a[k], phi = __umul64hi(a[k], a[k]);   // phi < 2^20
+    q0[k] = (uint32_t)plo; q1[k] = (uint32_t)(plo >> 32); q2[k] = (uint32_t)phi;
+    o0[k] = atoms_add(sa[k] + 8, q0[k]);
+  }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const uint32_t hi = (uint32_t)(a[k] >> 32) + carry_of(o[k], (uint32_t)a[k]);
+    if (hi) reds_add(sa[k] + 4, hi);
+  }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const unsigned long long m = (unsigned long long)q1[k] + carry_of(o0[k], q0[k]);
+    q1[k] = (uint32_t)m;
+    q2[k] += (uint32_t)(m >> 32);
+    o[k] = atoms_add(sa[k] + 12, q1[k]);
+  }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const uint32_t top = q2[k] + carry_of(o[k], q1[k]);
+    if (top) reds_add(sa[k] + 16, top);
+  }
+}
+
 // any other value: wide a (2^32 <= a < 2^42), or outside the integer window -> global sums
 __device__ __noinline__ void acc_slow(uint32_t sa, float v, float mult, double* S1g, double* S2g) {
   if (v == 0.0f) return;
@@ -331,6 +371,49 @@ __device__ __noinline__ float entry_any(const AccCtx& c, int j, float x, float s
   return xl;
 }
 
+// A quad with at least one value outside the one-word window (out of line: keeps the hot path
+// small).  All values at most two-word integers and x' >= 0.25 -> acc_quad_wide; else entry by
+// entry.  valid_mask bit k: entry k belongs to the segment.
+template <bool LOG, bool LIN>
+__device__ __noinline__ float4 quad_rare(const AccCtx& c, int4 jv, float4 xv, float scale,
+                                         uint32_t valid_mask, uint32_t spare_slot) {
+  const int j[4] = {jv.x, jv.y, jv.z, jv.w};
+  const float x[4] = {xv.x, xv.y, xv.z, xv.w};
+  float xn[4], xl[4], tl[4], tn[4];
+  bool ok = true;
+  uint32_t so[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const bool valid = (valid_mask >> k) & 1u;
+    xn[k] = __fmul_rn(x[k], scale);
+    xl[k] = log1p_ge_quarter(xn[k]);
+    ok = ok && (xn[k] >= 0.25f || !valid);
+    if (LOG) { tl[k] = xl[k] * c.mult_log; ok = ok && (in_window_wide(tl[k]) || !valid); }
+    if (LIN) { tn[k] = xn[k] * c.mult_lin; ok = ok && (in_window_wide(tn[k]) || !valid); }
+    const uint32_t slot = valid ? min((uint32_t)(j[k] - c.g0), c.last_slot) : spare_slot;
+    so[k] = slot * (kSetWords * 4u);
+  }
+  if (ok) {
+    if (LOG) {
+      unsigned long long al[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) al[k] = ((valid_mask >> k) & 1u) ? __float2ull_rz(tl[k]) : 0ull;
+      acc_quad_wide(c.sb_log, so, al);
+    }
+    if (LIN) {
+      unsigned long long an[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) an[k] = ((valid_mask >> k) & 1u) ? __float2ull_rz(tn[k]) : 0ull;
+      acc_quad_wide(c.sb_lin, so, an);
+    }
+  } else {
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if ((valid_mask >> k) & 1u) xl[k] = entry_any<LOG, LIN>(c, j[k], x[k], scale);
+  }
+  return make_float4(xl[0], xl[1], xl[2], xl[3]);
+}
+
 // ------------------------------------------------------------------ streaming kernel
 template <bool LOG, bool LIN>
 __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const FusedArgs a) {
@@ -349,8 +432,8 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
     while (grp + 1 < ng && (int)blockIdx.x >= plan->cta_first[grp + 1]) ++grp;
   }
   const float mult_log = plan->sc_log.mult, mult_lin = plan->sc_lin.mult;
-  const int f0 = grp * a.fine_per_group;
-  const int f1 = min(K, f0 + a.fine_per_group);
+  const int f0 = (grp * K) / plan->n_groups;              // group = blocks [grp K / ng, (grp + 1) K / ng)
+  const int f1 = ((grp + 1) * K) / plan->n_groups;
   const int g0 = f0 << RSC_SPLIT_SHIFT;
   const int ng_genes = min(a.n_cols, f1 << RSC_SPLIT_SHIFT) - g0;
   unsigned long long* counter = &a.plan->row_counter[grp];
@@ -379,7 +462,8 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
   };
 
   // One quad of 4 consecutive entries.  Straight-line code when every value is in the usual
-  // range (x' >= 0.25 and inside the integer windows), else entry by entry through entry_any.
+  // range (x' >= 0.25 and one-word integers), else through quad_rare (two-word integers, or
+  // entry by entry).
   // EDGE: only entries e0 + k in [0, len) belong to the segment; the others (a neighbouring
   // segment's) are neutralised by adding 0 to the spare slot Gt, so the code stays branch-free.
   auto quad = [&](auto edge_tag, const int4 jv, const float4 xv, float scale, int e0, int len) -> float4 {
@@ -411,9 +495,9 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
       if (LOG) acc_quad(sb_log, so, al);
       if (LIN) acc_quad(sb_lin, so, an);
     } else {
-#pragma unroll
-      for (int k = 0; k < 4; ++k)
-        if (valid[k]) xl[k] = entry_any<LOG, LIN>(cx, j[k], x[k], scale);
+      const uint32_t vm = (valid[0] ? 1u : 0u) | (valid[1] ? 2u : 0u) | (valid[2] ? 4u : 0u) |
+                          (valid[3] ? 8u : 0u);
+      return quad_rare<LOG, LIN>(cx, jv, xv, scale, vm, (uint32_t)Gt);
     }
     return make_float4(xl[0], xl[1], xl[2], xl[3]);
   };
@@ -586,8 +670,8 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_fp64_kernel(const 
     const int ng = plan->n_groups;
     while (grp + 1 < ng && (int)blockIdx.x >= plan->cta_first[grp + 1]) ++grp;
   }
-  const int f0 = grp * a.fine_per_group;
-  const int f1 = min(K, f0 + a.fine_per_group);
+  const int f0 = (grp * K) / plan->n_groups;              // group = blocks [grp K / ng, (grp + 1) K / ng)
+  const int f1 = ((grp + 1) * K) / plan->n_groups;
   const int g0 = f0 << RSC_SPLIT_SHIFT;
   const int ng_genes = min(a.n_cols, f1 << RSC_SPLIT_SHIFT) - g0;
   unsigned long long* counter = &a.plan->row_counter[grp];
@@ -740,7 +824,7 @@ int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i
       RSC_LAUNCH_CHECK("fused_tmax_kernel");
     }
     fused_plan_kernel<<<1, 1024, 0, st>>>(plan, X.n_cols, a.n_fine, a.fine_per_group, fused_grid(),
-                                          target_sum, gene_n_cells);
+                                          target_sum, (long long)X.n_rows, gene_n_cells);
     RSC_LAUNCH_CHECK("fused_plan_kernel");
     const size_t smem = (size_t)bytes_per_gene(which) * (size_t)a.Gt + 32;   // + the spare slot
     switch (which & 7) {
