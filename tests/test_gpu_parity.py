@@ -194,6 +194,22 @@ def test_hvg_select_same_inputs(G, seed, n_top, n_bins, log_flag):
     U.assert_hvg_matches(g, o, n_top, f"hvg G={G}", strict=False)
 
 
+def test_hvg_many_ties_takes_the_general_selection_path():
+    """5000 genes in one bin with only two distinct dispersions: 2500 equal z-scores sit in
+    the value bin that holds the cutoff -- more than the fast top-k path gathers -- so the
+    8-pass radix select runs; every tie at the cutoff is selected (reading R13 / H7)."""
+    from paper_2603_02402_b200 import rsc_hvg_select
+    G = 5000
+    mean = 1.0 + np.arange(G) / 8192.0                    # dyadic: var / mean is exactly 3 or 0.5
+    var = mean * np.where(np.arange(G) % 2 == 0, 3.0, 0.5)
+    for n_bins, log_flag in ((1, 1), (1, 0)):
+        o = O.hvg_select(mean, var, 100, n_bins, seurat_log=bool(log_flag))
+        g = rsc_hvg_select(torch.as_tensor(mean).cuda(), torch.as_tensor(var).cuda(), 100, n_bins, log_flag)
+        torch.cuda.synchronize()
+        U.assert_hvg_matches(g, o, 100, f"ties n_bins={n_bins} log={log_flag}", strict=False)
+        assert int(U.np_(g["count"])[0]) == int(o["mask"].sum()) == G // 2
+
+
 def test_hvg_golden_and_degenerate():
     from paper_2603_02402_b200 import rsc_hvg_select
     # hand-worked fixture (tests/golden/hvg_tiny.txt, case two_bins / single_gene_bin_and_tie)
