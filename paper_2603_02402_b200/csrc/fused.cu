@@ -43,7 +43,10 @@ namespace rsc {
 #define RSC_FU_THREADS 768
 #endif
 constexpr int kFuThreads = RSC_FU_THREADS;
-constexpr int kFuRowsPerGrab = 4;
+#ifndef RSC_FU_RG
+#define RSC_FU_RG 4
+#endif
+constexpr int kFuRowsPerGrab = RSC_FU_RG;
 constexpr int kMaxGroups = 64;
 constexpr int kSetWords = 5;               // u32 words per gene and moment set (w0 w1 s0 s1 s2)
 constexpr double kRowCost = 200.0;         // per-row-segment overhead, in entries (plan kernel)

@@ -22,7 +22,10 @@ namespace rsc {
 
 constexpr int kQcThreads = 1024;
 constexpr int kQcWarps = kQcThreads / 32;
-constexpr int kQcRowsPerGrab = 4;
+#ifndef RSC_QC_RG
+#define RSC_QC_RG 4
+#endif
+constexpr int kQcRowsPerGrab = RSC_QC_RG;
 #ifndef RSC_QC_AHEAD
 #define RSC_QC_AHEAD 4
 #endif
