@@ -380,3 +380,44 @@ def test_fixed_point_extreme_ranges():
             B.rsc_normalize_total(Xn, s, q["cell_total_i64"])
             mo, vo, _, _ = O.gene_moments(indptr, indices, U.np_(Xn.data), G, 0, 1)
             U.assert_moments_close(out["mean_lin"], out["var_lin"], mo, vo, f"lin s={s} which={which}")
+
+
+def test_edge_inputs_misaligned_explicit_zeros_and_empty():
+    """(a) indices / data at every 4-byte misalignment of the 16-byte quads (served by the generic
+    kernels): same results as the aligned streaming kernels; (b) explicit stored zeros are not
+    "detected" (reading R2) and stay zero through log1p; (c) a matrix of empty rows."""
+    from paper_2603_02402_b200 import binding as B, Csr
+    n, G, s = 300, 2100, 1e4
+    indptr, indices, data, _ = synth.small_nb_csr(n, G, 11, 0.5, empty_rows=(0, 299), empty_genes=(7,))
+    data = data.copy()
+    data[::17] = 0.0                                       # explicit zeros
+    flags = _flags(G, 11)
+    q_o = O.qc_metrics(indptr, indices, data, G, flags)
+    assert q_o["cell_n_genes"].sum() < len(data)           # the zeros are stored but not counted
+    ref = None
+    for off in range(4):
+        ib = torch.zeros(len(indices) + 8, dtype=torch.int32, device="cuda")
+        db = torch.zeros(len(data) + 8, dtype=torch.float32, device="cuda")
+        iv, dv = ib[off:off + len(indices)], db[off:off + len(data)]
+        iv.copy_(torch.as_tensor(indices)); dv.copy_(torch.as_tensor(data))
+        X = Csr(torch.as_tensor(indptr).cuda(), iv, dv, G)
+        q = B.rsc_qc_metrics(X, torch.as_tensor(flags).cuda())
+        for k in ("cell_total_i64", "cell_n_genes", "cell_flag_total_i64", "gene_n_cells", "gene_total_i64"):
+            U.assert_int_equal(q[k], q_o[k], f"{k} off={off}")
+        out = B.rsc_normalize_log1p_moments(X, s, q["cell_total_i64"], q["gene_n_cells"], 3, 1)
+        xl = U.np_(X.data)
+        assert np.all((xl == 0) == (data == 0))
+        mo, vo, _, _ = O.gene_moments(indptr, indices, xl, G, 0, 1)
+        U.assert_moments_close(out["mean_log"], out["var_log"], mo, vo, f"log off={off}")
+        if ref is None:
+            ref = xl.copy()
+        else:
+            assert np.array_equal(xl, ref), "aligned and misaligned paths write different x''"
+        assert float(db[:off].abs().sum()) == 0 and float(db[off + len(data):].abs().sum()) == 0
+    # (c) only empty rows
+    X = Csr(torch.zeros(6, dtype=torch.int64, device="cuda"), torch.zeros(0, dtype=torch.int32, device="cuda"),
+            torch.zeros(0, dtype=torch.float32, device="cuda"), 50)
+    q = B.rsc_qc_metrics(X)
+    assert int(q["cell_total_i64"].abs().sum()) == 0 and int(q["gene_n_cells"].abs().sum()) == 0
+    out = B.rsc_normalize_log1p_moments(X, s, q["cell_total_i64"], q["gene_n_cells"], 3, 1)
+    assert float(out["mean_log"].abs().sum()) == 0 and float(out["var_lin"].abs().sum()) == 0
