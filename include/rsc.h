@@ -109,6 +109,17 @@ int rsc_qc_metrics(const rsc_csr* X, const uint8_t* gene_flags,
                    int64_t* cell_flag_total_i64, float* cell_flag_pct,
                    int32_t* gene_n_cells, int64_t* gene_total_i64, uint32_t* row_splits,
                    void* ws, size_t ws_bytes, void* stream);
+/* The same call, but only the row_splits entries whose block index k is listed in
+ * split_blocks (a HOST array of n_split_blocks <= 32 indices in [0, K]) are written; the other
+ * entries of the table are left untouched.  The fused pass reads just a few entries per row
+ * (rsc_moments_split_blocks tells which), and emitting only those spares the QC pass most of
+ * the table's cost.  n_split_blocks = 0 -> the full table, as rsc_qc_metrics. */
+int rsc_qc_metrics_splits(const rsc_csr* X, const uint8_t* gene_flags,
+                          int64_t* cell_total_i64, float* cell_total_f32, int32_t* cell_n_genes,
+                          int64_t* cell_flag_total_i64, float* cell_flag_pct,
+                          int32_t* gene_n_cells, int64_t* gene_total_i64, uint32_t* row_splits,
+                          const int32_t* split_blocks, int32_t n_split_blocks,
+                          void* ws, size_t ws_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------------
  * rsc_normalize_total — PAPER.md:L91  x'_ij = (x_ij / sum_j x_ij) * s, in place.
@@ -172,6 +183,10 @@ int rsc_gene_moments(const rsc_csr* X, int transform, int ddof,
 #define RSC_MOMENTS_LIN 2
 #define RSC_MOMENTS_FP64_ACC 4
 size_t rsc_normalize_log1p_moments_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
+/* Block indices k of the row split table that rsc_normalize_log1p_moments reads for this
+ * n_cols / which_moments (the edges of its gene-range groups), written to blocks_out[0..cap);
+ * returns their number (0 when the call would not use a table; > cap -> nothing written). */
+int32_t rsc_moments_split_blocks(int32_t n_cols, int which_moments, int32_t* blocks_out, int32_t cap);
 int rsc_normalize_log1p_moments(rsc_csr* X, float target_sum, const int64_t* cell_total_i64,
                                 const int32_t* gene_n_cells, const uint32_t* row_splits,
                                 int which_moments, int ddof,

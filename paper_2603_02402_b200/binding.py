@@ -32,7 +32,8 @@ RSC_HVG_SEURAT_LOG = 1
 EXPORTS = [
     "rsc_last_error", "rsc_version", "rsc_kernel_launch_count",
     "rsc_row_splits_count", "rsc_row_splits", "rsc_set_option",
-    "rsc_qc_metrics_workspace_bytes", "rsc_qc_metrics",
+    "rsc_qc_metrics_workspace_bytes", "rsc_qc_metrics", "rsc_qc_metrics_splits",
+    "rsc_moments_split_blocks",
     "rsc_normalize_total", "rsc_log1p",
     "rsc_gene_moments_workspace_bytes", "rsc_gene_moments",
     "rsc_normalize_log1p_moments_workspace_bytes", "rsc_normalize_log1p_moments",
@@ -104,6 +105,9 @@ def lib() -> C.CDLL:
     L.rsc_row_splits_count.argtypes = [i64, i32]
     L.rsc_row_splits.argtypes = [p, p, p]
     L.rsc_qc_metrics.argtypes = [p] + [p] * 9 + [p, sz, p]
+    L.rsc_qc_metrics_splits.argtypes = [p] + [p] * 9 + [p, i32, p, sz, p]
+    L.rsc_moments_split_blocks.argtypes = [i32, C.c_int, p, i32]
+    L.rsc_moments_split_blocks.restype = i32
     L.rsc_normalize_total.argtypes = [p, flt, p, p, p]
     L.rsc_log1p.argtypes = [p, p]
     L.rsc_gene_moments.argtypes = [p, C.c_int, C.c_int, p, p, p, p, p, sz, p]
@@ -198,8 +202,15 @@ def rsc_row_splits(X: Csr, stream=None) -> torch.Tensor:
     return out
 
 
+def rsc_moments_split_blocks(n_cols: int, which_moments: int) -> list:
+    """Block indices of the row split table that rsc_normalize_log1p_moments reads."""
+    buf = (C.c_int32 * 80)()
+    k = lib().rsc_moments_split_blocks(n_cols, which_moments, C.cast(buf, C.c_void_p), 80)
+    return [int(buf[i]) for i in range(min(k, 80))]
+
+
 def rsc_qc_metrics(X: Csr, gene_flags: Optional[torch.Tensor] = None, stream=None,
-                   with_row_splits: bool = False) -> dict:
+                   with_row_splits: bool = False, split_blocks: Optional[list] = None) -> dict:
     _need_cuda(X)
     L, dev, n, G = lib(), X.device, X.n_rows, X.n_cols
     out = dict(
@@ -217,9 +228,16 @@ def rsc_qc_metrics(X: Csr, gene_flags: Optional[torch.Tensor] = None, stream=Non
     splits = None
     if with_row_splits and X.sorted_indices:
         splits = torch.empty(max(1, rsc_row_splits_count(n, G)), dtype=torch.int32, device=dev)
-    _check(L.rsc_qc_metrics(C.byref(cs), _ptr(gene_flags), *[_ptr(out[k]) for k in (
-        "cell_total_i64", "cell_total_f32", "cell_n_genes", "cell_flag_total_i64", "cell_flag_pct",
-        "gene_n_cells", "gene_total_i64")], _ptr(splits), _ptr(ws), ws.numel(), _stream(stream)))
+    outs = [_ptr(out[k]) for k in ("cell_total_i64", "cell_total_f32", "cell_n_genes",
+                                   "cell_flag_total_i64", "cell_flag_pct", "gene_n_cells", "gene_total_i64")]
+    if split_blocks:
+        sb = (C.c_int32 * len(split_blocks))(*split_blocks)
+        _check(L.rsc_qc_metrics_splits(C.byref(cs), _ptr(gene_flags), *outs, _ptr(splits),
+                                       C.cast(sb, C.c_void_p), len(split_blocks), _ptr(ws), ws.numel(),
+                                       _stream(stream)))
+    else:
+        _check(L.rsc_qc_metrics(C.byref(cs), _ptr(gene_flags), *outs, _ptr(splits), _ptr(ws), ws.numel(),
+                                _stream(stream)))
     if splits is not None:
         out["row_splits"] = splits
     return out
@@ -381,11 +399,16 @@ class Preprocessor:
         w0, w1, w2, sp = self._stage_ws
         if events:
             events[0].record(st)
-        _check(L.rsc_qc_metrics(C.byref(cs), _ptr(gene_flags), _ptr(o["cell_total_i64"]),
-                                _ptr(o["cell_total_f32"]), _ptr(o["cell_n_genes"]),
-                                _ptr(o["cell_flag_total_i64"]), _ptr(o["cell_flag_pct"]),
-                                _ptr(o["gene_n_cells"]), _ptr(o["gene_total_i64"]), _ptr(sp),
-                                _ptr(w0), w0.numel(), sp_))
+        if not hasattr(self, "_need"):                     # split entries the fused pass reads
+            nb = rsc_moments_split_blocks(X.n_cols, p.which_moments)
+            nb = nb if 0 < len(nb) <= 32 else []
+            self._need = (C.c_int32 * max(1, len(nb)))(*nb), len(nb)
+        _check(L.rsc_qc_metrics_splits(C.byref(cs), _ptr(gene_flags), _ptr(o["cell_total_i64"]),
+                                       _ptr(o["cell_total_f32"]), _ptr(o["cell_n_genes"]),
+                                       _ptr(o["cell_flag_total_i64"]), _ptr(o["cell_flag_pct"]),
+                                       _ptr(o["gene_n_cells"]), _ptr(o["gene_total_i64"]), _ptr(sp),
+                                       C.cast(self._need[0], C.c_void_p), self._need[1],
+                                       _ptr(w0), w0.numel(), sp_))
         if events:
             events[1].record(st)
         _check(L.rsc_normalize_log1p_moments(

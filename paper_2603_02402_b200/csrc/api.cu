@@ -130,19 +130,39 @@ int rsc_row_splits(const rsc_csr* X, uint32_t* row_splits, void* stream) {
   return launch_row_splits(*X, row_splits, static_cast<cudaStream_t>(stream));
 }
 
-int rsc_qc_metrics(const rsc_csr* X, const uint8_t* gene_flags, int64_t* cell_total_i64,
-                   float* cell_total_f32, int32_t* cell_n_genes, int64_t* cell_flag_total_i64,
-                   float* cell_flag_pct, int32_t* gene_n_cells, int64_t* gene_total_i64,
-                   uint32_t* row_splits, void* ws, size_t ws_bytes, void* stream) {
+int rsc_qc_metrics_splits(const rsc_csr* X, const uint8_t* gene_flags, int64_t* cell_total_i64,
+                          float* cell_total_f32, int32_t* cell_n_genes, int64_t* cell_flag_total_i64,
+                          float* cell_flag_pct, int32_t* gene_n_cells, int64_t* gene_total_i64,
+                          uint32_t* row_splits, const int32_t* split_blocks, int32_t n_split_blocks,
+                          void* ws, size_t ws_bytes, void* stream) {
   int rc = check_csr(X, "rsc_qc_metrics", true);
   if (rc) return rc;
+  RSC_CHECK_ARG(n_split_blocks >= 0 && n_split_blocks <= 32, "rsc_qc_metrics: n_split_blocks must be in [0, 32]");
+  RSC_CHECK_ARG(n_split_blocks == 0 || split_blocks != nullptr, "rsc_qc_metrics: split_blocks is NULL");
+  for (int i = 0; i < n_split_blocks; ++i)
+    RSC_CHECK_ARG(split_blocks[i] >= 0 && split_blocks[i] <= ::rsc::split_blocks(X->n_cols),
+                  "rsc_qc_metrics: split_blocks[%d] out of range", i);
   if ((rc = check_device())) return rc;
   if ((rc = check_ws("rsc_qc_metrics", ws, ws_bytes, qc_workspace_bytes(X->n_rows, X->n_cols, X->nnz))))
     return rc;
   if (!(X->flags & RSC_CSR_SORTED)) row_splits = nullptr;
   return launch_qc(*X, gene_flags, cell_total_i64, cell_total_f32, cell_n_genes,
-                   cell_flag_total_i64, cell_flag_pct, gene_n_cells, gene_total_i64, row_splits, ws,
-                   ws_bytes, static_cast<cudaStream_t>(stream));
+                   cell_flag_total_i64, cell_flag_pct, gene_n_cells, gene_total_i64, row_splits,
+                   split_blocks, n_split_blocks, ws, ws_bytes, static_cast<cudaStream_t>(stream));
+}
+
+int rsc_qc_metrics(const rsc_csr* X, const uint8_t* gene_flags, int64_t* cell_total_i64,
+                   float* cell_total_f32, int32_t* cell_n_genes, int64_t* cell_flag_total_i64,
+                   float* cell_flag_pct, int32_t* gene_n_cells, int64_t* gene_total_i64,
+                   uint32_t* row_splits, void* ws, size_t ws_bytes, void* stream) {
+  return rsc_qc_metrics_splits(X, gene_flags, cell_total_i64, cell_total_f32, cell_n_genes,
+                               cell_flag_total_i64, cell_flag_pct, gene_n_cells, gene_total_i64,
+                               row_splits, nullptr, 0, ws, ws_bytes, stream);
+}
+
+int32_t rsc_moments_split_blocks(int32_t n_cols, int which_moments, int32_t* blocks_out, int32_t cap) {
+  if (n_cols <= 0 || blocks_out == nullptr || cap < 0) return 0;
+  return fused_split_blocks(n_cols, which_moments, blocks_out, cap);
 }
 
 int rsc_normalize_total(rsc_csr* X, float target_sum, const int64_t* cell_total_i64,

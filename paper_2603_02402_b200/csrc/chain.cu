@@ -79,9 +79,13 @@ static int run_chain(rsc_csr* X, const uint8_t* gene_flags, const rsc_params* pr
   double* var_lin = out->var_lin ? out->var_lin : w.var_lin;
 
   uint32_t* splits = (X->flags & RSC_CSR_SORTED) ? w.splits : nullptr;
+  // only the split entries the fused pass will read (its group edges) are produced
+  int32_t need[32];
+  int32_t n_need = fused_split_blocks(X->n_cols, prm->which_moments, need, 32);
+  if (n_need > 32) n_need = 0;
   int rc = launch_qc(*X, gene_flags, cell_total, out->cell_total_f32, out->cell_n_genes,
                      out->cell_flag_total_i64, out->cell_flag_pct, gene_n_cells,
-                     out->gene_total_i64, splits, w.qc_ws, w.qc_bytes, st);
+                     out->gene_total_i64, splits, need, n_need, w.qc_ws, w.qc_bytes, st);
   if (rc) return rc;
   rc = launch_fused(*X, prm->target_sum, cell_total, gene_n_cells, splits, prm->which_moments, prm->ddof,
                     mean_log, var_log, mean_lin, var_lin, nullptr, w.fused_ws, w.fused_bytes, st);

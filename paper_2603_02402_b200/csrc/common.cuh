@@ -69,7 +69,10 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 int launch_qc(const rsc_csr& X, const uint8_t* gene_flags, int64_t* cell_total_i64,
               float* cell_total_f32, int32_t* cell_n_genes, int64_t* cell_flag_total_i64,
               float* cell_flag_pct, int32_t* gene_n_cells, int64_t* gene_total_i64,
-              uint32_t* row_splits, void* ws, size_t ws_bytes, cudaStream_t st);
+              uint32_t* row_splits, const int32_t* split_blocks, int32_t n_split_blocks, void* ws,
+              size_t ws_bytes, cudaStream_t st);
+// column-block indices at which the fused pass cuts the gene axis (edges of its groups)
+int fused_split_blocks(int32_t n_cols, int which, int32_t* out, int32_t cap);
 size_t qc_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
 int launch_row_splits(const rsc_csr& X, uint32_t* splits, cudaStream_t st);
 

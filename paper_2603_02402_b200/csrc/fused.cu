@@ -766,6 +766,17 @@ static bool fused_fast_ok(const rsc_csr& X, int which) {
   return ng <= kMaxGroups && ng <= fused_grid();
 }
 
+// the row split entries the streaming kernel reads: the edges (c K) / ng of its groups
+int fused_split_blocks(int32_t n_cols, int which, int32_t* out, int32_t cap) {
+  const int fpg = fine_per_group(n_cols, which);
+  if (fpg < 1 || (which & 3) == 0) return 0;
+  const int K = split_blocks(n_cols);
+  const int ng = (K + fpg - 1) / fpg;
+  if (ng + 1 > cap) return ng + 1;
+  for (int c = 0; c <= ng; ++c) out[c] = (c * K) / ng;
+  return ng + 1;
+}
+
 size_t fused_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t) {
   const size_t K1 = (size_t)split_blocks(n_cols) + 1;
   return 4 * align_up(sizeof(double) * (size_t)n_cols, 256) + align_up(sizeof(FusedPlan), 256) +

@@ -51,6 +51,8 @@ struct QcArgs {
   int32_t* gene_n_cells;
   unsigned long long* gene_total;
   uint32_t* splits;
+  int32_t n_need;            // > 0: only the split entries need[0..n_need) are written
+  int32_t need[32];
   unsigned long long* row_counter;
 };
 
@@ -234,10 +236,14 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
         if (SPLITS) {
           // split table of the row: lane k finds #{entries with column < k * RSC_SPLIT_WIDTH} by
           // binary search in the (sorted) row, whose lines were just streamed (L2 / L1 hits)
-          for (int k = lane; k <= K; k += 32) {
+          // (all K + 1 entries, or only the listed ones: fewer probing lanes, less re-read traffic)
+          const int nk = a.n_need > 0 ? a.n_need : K + 1;
+          for (int i = lane; i < nk; i += 32) {
+            const int k = a.n_need > 0 ? a.need[i] : i;
             const int32_t bound = k << RSC_SPLIT_SHIFT;
             int lo = 0, hi = len;
             if (k == 0) hi = 0;
+            else if (k >= K) lo = len;
             while (lo < hi) {
               const int mid = (lo + hi) >> 1;
               if (__ldg(a.indices + beg + mid) < bound) lo = mid + 1; else hi = mid;
@@ -328,7 +334,8 @@ int launch_qc_generic(const rsc_csr&, const uint8_t*, int64_t*, float*, int32_t*
 int launch_qc(const rsc_csr& X, const uint8_t* gene_flags, int64_t* cell_total_i64,
               float* cell_total_f32, int32_t* cell_n_genes, int64_t* cell_flag_total_i64,
               float* cell_flag_pct, int32_t* gene_n_cells, int64_t* gene_total_i64,
-              uint32_t* row_splits, void* ws, size_t, cudaStream_t st) {
+              uint32_t* row_splits, const int32_t* need_blocks, int32_t n_need_blocks, void* ws,
+              size_t, cudaStream_t st) {
   // the 128-bit loads need 16-byte aligned arrays; anything else takes the generic kernel
   const bool aligned = ((reinterpret_cast<uintptr_t>(X.indices) | reinterpret_cast<uintptr_t>(X.data)) & 15) == 0;
   if (!aligned || g_opt.force_generic || X.n_cols > kQcMaxGenes) {
@@ -354,6 +361,11 @@ int launch_qc(const rsc_csr& X, const uint8_t* gene_flags, int64_t* cell_total_i
   a.gene_n_cells = gene_n_cells;
   a.gene_total = reinterpret_cast<unsigned long long*>(gene_total_i64);
   a.splits = row_splits;
+  a.n_need = 0;
+  if (need_blocks != nullptr && n_need_blocks > 0 && n_need_blocks <= 32) {
+    a.n_need = n_need_blocks;
+    for (int i = 0; i < n_need_blocks; ++i) a.need[i] = need_blocks[i];
+  }
   a.row_counter = static_cast<unsigned long long*>(ws);
   static bool attr_set = false;
   if (!attr_set) {

@@ -281,6 +281,22 @@ def test_row_splits_qc_and_standalone(n, G, seed, depth, er, eg):
     b = U.np_(q["row_splits"]).astype(np.int64)[: want.size].reshape(want.shape)
     assert np.array_equal(a, want), "rsc_row_splits"
     assert np.array_equal(b, want), "row splits emitted by rsc_qc_metrics"
+    # only the entries the fused pass reads (rsc_qc_metrics_splits): the listed columns of the
+    # table are exact, and the fused pass fed with that partial table gives the same moments
+    for which in (1, 3):
+        need = B.rsc_moments_split_blocks(G, which)
+        K = want.shape[1] - 1
+        assert need and need[0] == 0 and need[-1] == K and need == sorted(set(need))
+        qp = B.rsc_qc_metrics(X, None, with_row_splits=True, split_blocks=need)
+        c = U.np_(qp["row_splits"]).astype(np.int64)[: want.size].reshape(want.shape)
+        assert np.array_equal(c[:, need], want[:, need]), "partial row split table"
+        X1, X2 = U.clone(X), U.clone(X)
+        o1 = B.rsc_normalize_log1p_moments(X1, 1e4, q["cell_total_i64"], q["gene_n_cells"], which, 0,
+                                           row_splits=q["row_splits"], return_sums=True)
+        o2 = B.rsc_normalize_log1p_moments(X2, 1e4, q["cell_total_i64"], q["gene_n_cells"], which, 0,
+                                           row_splits=qp["row_splits"], return_sums=True)
+        assert torch.equal(X1.data, X2.data)
+        np.testing.assert_allclose(U.np_(o1["sums"]), U.np_(o2["sums"]), rtol=1e-14)
 
 
 @pytest.fixture
