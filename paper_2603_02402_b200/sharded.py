@@ -50,6 +50,12 @@ def global_cell_count(n_local: int, device, group=None) -> int:
     return int(t[0])
 
 
+def _need_blocks(n_cols: int, which_moments: int):
+    nb = B.rsc_moments_split_blocks(n_cols, which_moments)
+    nb = nb if 0 < len(nb) <= 32 else []
+    return (C.c_int32 * max(1, len(nb)))(*nb), len(nb)
+
+
 def preprocess_sharded(pp: "B.Preprocessor", X: "B.Csr", gene_flags: Optional[torch.Tensor],
                        events=None, group=None) -> dict:
     """QC -> all-reduce -> fused pass (raw sums) -> all-reduce -> finalize -> HVG.
@@ -68,16 +74,18 @@ def preprocess_sharded(pp: "B.Preprocessor", X: "B.Csr", gene_flags: Optional[to
             w2=B._ws(L.rsc_hvg_select_workspace_bytes(G, p.n_bins), X.device),
             splits=(torch.empty(max(1, B.rsc_row_splits_count(n, G)), dtype=torch.int32,
                                 device=X.device) if X.sorted_indices else None),
+            need=_need_blocks(G, p.which_moments),        # split entries the fused pass reads
             sums=torch.zeros(4, G, dtype=torch.float64, device=X.device),
             n_total=global_cell_count(n, X.device, group))
     sh = pp._sh
     if events:
         events[0].record(st)
-    B._check(L.rsc_qc_metrics(C.byref(cs), B._ptr(gene_flags), B._ptr(o["cell_total_i64"]),
-                              B._ptr(o["cell_total_f32"]), B._ptr(o["cell_n_genes"]),
-                              B._ptr(o["cell_flag_total_i64"]), B._ptr(o["cell_flag_pct"]),
-                              B._ptr(o["gene_n_cells"]), B._ptr(o["gene_total_i64"]),
-                              B._ptr(sh["splits"]), B._ptr(sh["w0"]), sh["w0"].numel(), sp))
+    B._check(L.rsc_qc_metrics_splits(C.byref(cs), B._ptr(gene_flags), B._ptr(o["cell_total_i64"]),
+                                     B._ptr(o["cell_total_f32"]), B._ptr(o["cell_n_genes"]),
+                                     B._ptr(o["cell_flag_total_i64"]), B._ptr(o["cell_flag_pct"]),
+                                     B._ptr(o["gene_n_cells"]), B._ptr(o["gene_total_i64"]),
+                                     B._ptr(sh["splits"]), C.cast(sh["need"][0], C.c_void_p),
+                                     sh["need"][1], B._ptr(sh["w0"]), sh["w0"].numel(), sp))
     allreduce_gene_stats({"n_cells": o["gene_n_cells"], "total": o["gene_total_i64"]}, {}, group)
     if events:
         events[1].record(st)
