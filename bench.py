@@ -29,8 +29,8 @@ NOMINAL_HBM_GBS = 8000.0          # BASELINE.json's denominator ("fraction of 8 
 FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 BYTES_PER_NNZ = {"qc": 8.0, "fused": 12.0, "chain": 20.0}   # SURVEY.md §8(d), DESIGN.md §7
 # dram__bytes_read.sum + dram__bytes_write.sum of one fused-pass launch, from the ncu --set full
-# capture in profiles/r01b_cfg3.md; key = (config, which_moments), full-size runs only
-NCU_TRAFFIC_BYTES = {(3, 1): 12.440818e9 + 5.897024e9}
+# capture in profiles/r01c_cfg3.md; key = (config, which_moments), full-size runs only
+NCU_TRAFFIC_BYTES = {(3, 1): 12.336356e9 + 5.890303e9}
 
 
 def parse_args():
@@ -288,7 +288,7 @@ def main():
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "peak_source": peak_src,
                 "traffic": NCU_TRAFFIC_BYTES.get((args.config, args.which_moments)) if args.cells is None else None,
-                "traffic_source": "profiles/r01b_cfg3.md (ncu --set full, bytes per launch)",
+                "traffic_source": "profiles/r01c_cfg3.md (ncu --set full, bytes per launch)",
                 "algorithmic_bytes_per_nnz": BYTES_PER_NNZ["fused"],
                 "ms_per_launch": fused_ms, "frac_of_8TBs": achieved / NOMINAL_HBM_GBS}
     stages = {
