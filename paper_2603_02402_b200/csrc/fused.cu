@@ -27,8 +27,9 @@
 //     only receive carries: ~3.1 atomics per entry and set.  a >= 2^32 takes the same path
 //     with 64-bit a (a < 2^42 by construction); v below the window (or negative / NaN) goes
 //     to the global double sums directly.  Integer adds commute, so the sums are exact and
-//     independent of the order of the adds; they are converted to double once per flush
-//     (every <= 4092 rows, so no word can overflow).
+//     independent of the order of the adds; a flush (every <= 4092 rows, so no word can
+//     overflow) adds every word to its own 64-bit global counter, converted to double once at
+//     the end (fused_finish_kernel): bit-reproducible moments.
 //   * RSC_MOMENTS_FP64_ACC selects plain double accumulators (CAS atomics) instead: any
 //     value range, slower (fused_stream_fp64_kernel).
 #include <math.h>
@@ -83,6 +84,8 @@ struct FusedArgs {
   float target_sum;
   uint32_t row_budget;       // a CTA stops grabbing rows once it has taken this many (then flushes)
   double* S1log; double* S2log; double* S1lin; double* S2lin;
+  unsigned long long* acc_log;   // [5][n_cols] global totals of the words w0 w1 s0 s1 s2
+  unsigned long long* acc_lin;
   FusedPlan* plan;
 };
 
@@ -636,7 +639,7 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
       rnext = __shfl_sync(0xffffffffu, pending, 0);
     }
     done = __syncthreads_or(saw_end);
-    // flush this CTA's accumulators into the global double sums and clear them
+    // flush this CTA's accumulators into the global integer totals and clear them
     for (int s = tid; s < ng_genes; s += kFuThreads) {
       const int g = g0 + s;
 #pragma unroll
@@ -645,12 +648,17 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
         uint32_t* w = fsm + ((size_t)set * Gt + s) * kSetWords;
         const uint32_t w0 = w[0], w1 = w[1], s0 = w[2], s1 = w[3], s2 = w[4];
         if (w0 | w1 | s0 | s1 | s2) {
-          const MomentScale& sc = is_log ? plan->sc_log : plan->sc_lin;
-          const double v1 = (double)(((unsigned long long)w1 << 32) | w0) * sc.inv1;
-          const double v2 = ((double)s2 * 18446744073709551616.0 +
-                             (double)(((unsigned long long)s1 << 32) | s0)) * sc.inv2;
-          atomicAdd(is_log ? &a.S1log[g] : &a.S1lin[g], v1);
-          atomicAdd(is_log ? &a.S2log[g] : &a.S2lin[g], v2);
+          // integer totals in global memory: every 32-bit word of the CTA's sums is added to
+          // its own 64-bit counter (no carries between counters, so plain fire-and-forget
+          // atomics; a counter overflows only after 2^32 flushes): exact, and independent of
+          // the CTA order and of the grid
+          unsigned long long* acc = (is_log ? a.acc_log : a.acc_lin) + g;
+          const size_t G64 = (size_t)a.n_cols;
+          if (w0) atomicAdd(acc, (unsigned long long)w0);
+          if (w1) atomicAdd(acc + G64, (unsigned long long)w1);
+          if (s0) atomicAdd(acc + 2 * G64, (unsigned long long)s0);
+          if (s1) atomicAdd(acc + 3 * G64, (unsigned long long)s1);
+          if (s2) atomicAdd(acc + 4 * G64, (unsigned long long)s2);
           w[0] = 0u; w[1] = 0u; w[2] = 0u; w[3] = 0u; w[4] = 0u;
         }
       }
@@ -730,6 +738,29 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_fp64_kernel(const 
   } while (!done);
 }
 
+// ------------------------------------------------------------------ integer totals -> sums, moments
+// S += total * 2^-k (S holds what the out-of-window values added directly, usually 0), then
+// mean = S1 / n, var = max(0, (S2 - n mean^2) / (n - ddof)) as rsc_moments_finalize
+__global__ void __launch_bounds__(256)
+fused_finish_kernel(int G, double n, double denom, const FusedPlan* __restrict__ plan, int is_lin,
+                    const unsigned long long* __restrict__ acc, double* __restrict__ S1,
+                    double* __restrict__ S2, double* __restrict__ mean, double* __restrict__ var) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= G) return;
+  const MomentScale sc = is_lin ? plan->sc_lin : plan->sc_log;
+  const double two32 = 4294967296.0;
+  const size_t Gs = (size_t)G;
+  const double t1 = (double)acc[Gs + g] * two32 + (double)acc[g];
+  const double t2 = ((double)acc[4 * Gs + g] * two32 + (double)acc[3 * Gs + g]) * two32 + (double)acc[2 * Gs + g];
+  const double s1 = S1[g] + t1 * sc.inv1, s2 = S2[g] + t2 * sc.inv2;
+  S1[g] = s1;
+  S2[g] = s2;
+  const double m = s1 / n;
+  const double v = (s2 - n * m * m) / denom;
+  if (mean) mean[g] = m;
+  if (var) var[g] = v > 0.0 ? v : (v == v ? 0.0 : v);
+}
+
 // ------------------------------------------------------------------ host side
 int launch_fused_generic(const rsc_csr&, float, const int64_t*, int, double*, double*, double*,
                          double*, cudaStream_t);
@@ -780,7 +811,8 @@ int fused_split_blocks(int32_t n_cols, int which, int32_t* out, int32_t cap) {
 size_t fused_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t) {
   const size_t K1 = (size_t)split_blocks(n_cols) + 1;
   return 4 * align_up(sizeof(double) * (size_t)n_cols, 256) + align_up(sizeof(FusedPlan), 256) +
-         align_up(sizeof(uint32_t) * (size_t)n_rows * K1, 256);
+         align_up(sizeof(uint32_t) * (size_t)n_rows * K1, 256) +
+         2 * align_up(5 * sizeof(unsigned long long) * (size_t)n_cols, 256);
 }
 
 template <typename Kern>
@@ -807,17 +839,19 @@ int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i
     rc = launch_fused_generic(X, target_sum, cell_total_i64, which, S1log, S2log, S1lin, S2lin, st);
     if (rc != RSC_OK) return rc;
   } else {
-    if (which & RSC_MOMENTS_LOG) {
-      RSC_CUDA(cudaMemsetAsync(S1log, 0, sizeof(double) * G, st));
-      RSC_CUDA(cudaMemsetAsync(S2log, 0, sizeof(double) * G, st));
+    // workspace: 4 double sums | 2 x 5 integer totals | plan | (row split table); the sums, the
+    // totals and the plan (tmax) start from zero: one memset when the sums live in the workspace
+    const size_t asz = align_up(5 * sizeof(unsigned long long) * G, 256);
+    unsigned char* accb = w + 4 * gsz;
+    FusedPlan* plan = reinterpret_cast<FusedPlan*>(accb + 2 * asz);
+    if (sums_out == nullptr) {
+      RSC_CUDA(cudaMemsetAsync(w, 0, 4 * gsz + 2 * asz + sizeof(FusedPlan), st));
+    } else {
+      RSC_CUDA(cudaMemsetAsync(sums_out, 0, 4 * sizeof(double) * G, st));
+      RSC_CUDA(cudaMemsetAsync(accb, 0, 2 * asz + sizeof(FusedPlan), st));
     }
-    if (which & RSC_MOMENTS_LIN) {
-      RSC_CUDA(cudaMemsetAsync(S1lin, 0, sizeof(double) * G, st));
-      RSC_CUDA(cudaMemsetAsync(S2lin, 0, sizeof(double) * G, st));
-    }
-    FusedPlan* plan = reinterpret_cast<FusedPlan*>(w + 4 * gsz);
     if (row_splits == nullptr) {
-      uint32_t* sp = reinterpret_cast<uint32_t*>(w + 4 * gsz + align_up(sizeof(FusedPlan), 256));
+      uint32_t* sp = reinterpret_cast<uint32_t*>(accb + 2 * asz + align_up(sizeof(FusedPlan), 256));
       if ((rc = launch_row_splits(X, sp, st)) != RSC_OK) return rc;
       row_splits = sp;
     }
@@ -829,7 +863,9 @@ int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i
     a.splits = row_splits; a.target_sum = target_sum;
     a.row_budget = (uint32_t)g_opt.fused_row_budget;
     a.S1log = S1log; a.S2log = S2log; a.S1lin = S1lin; a.S2lin = S2lin; a.plan = plan;
-    RSC_CUDA(cudaMemsetAsync(&plan->tmax, 0, sizeof(unsigned long long), st));
+    const bool int_acc = !(which & RSC_MOMENTS_FP64_ACC);
+    a.acc_log = reinterpret_cast<unsigned long long*>(accb);
+    a.acc_lin = reinterpret_cast<unsigned long long*>(accb + asz);
     {
       int64_t blocks = (X.n_rows + 255) / 256;
       const int64_t cap = (int64_t)sm_count() * 4;
@@ -850,6 +886,21 @@ int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i
       default: rc = launch_stream(fused_stream_fp64_kernel<true, true>, a, smem, st); break;
     }
     if (rc != RSC_OK) return rc;
+    if (int_acc) {
+      const unsigned blocks = (unsigned)((G + 255) / 256);
+      const double n = (double)X.n_rows, denom = (double)(X.n_rows - ddof);
+      if (which & RSC_MOMENTS_LOG) {
+        fused_finish_kernel<<<blocks, 256, 0, st>>>(X.n_cols, n, denom, plan, 0, a.acc_log, S1log, S2log,
+                                                    mean_log, var_log);
+        RSC_LAUNCH_CHECK("fused_finish_kernel");
+      }
+      if (which & RSC_MOMENTS_LIN) {
+        fused_finish_kernel<<<blocks, 256, 0, st>>>(X.n_cols, n, denom, plan, 1, a.acc_lin, S1lin, S2lin,
+                                                    mean_lin, var_lin);
+        RSC_LAUNCH_CHECK("fused_finish_kernel");
+      }
+      return RSC_OK;
+    }
   }
   if (which & RSC_MOMENTS_LOG) {
     rc = finalize_moments(X.n_cols, X.n_rows, ddof, S1log, S2log, mean_log, var_log, st);

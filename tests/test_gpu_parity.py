@@ -340,8 +340,8 @@ def test_streaming_kernels_flush_paths(small_budgets, n, G, seed, depth, er, eg,
 
 def test_fused_equals_unfused_bitwise_and_is_order_independent():
     """The fused pass writes the very x'' that rsc_normalize_total + rsc_log1p write, and its
-    on-chip fixed-point sums do not depend on the order of the atomic adds; only the few
-    per-CTA partial sums are added to the global doubles in scheduling order (last-bit noise)."""
+    integer sums (on chip and in global memory) do not depend on the order of the atomic adds, the
+    CTA schedule or the grid: the moments are bit-reproducible."""
     from paper_2603_02402_b200 import binding as B
     indptr, indices, data, _ = synth.small_nb_csr(1500, 4099, 3, 0.4)
     X = U.to_dev(indptr, indices, data, 4099)
@@ -357,12 +357,14 @@ def test_fused_equals_unfused_bitwise_and_is_order_independent():
         out2 = B.rsc_normalize_log1p_moments(X2, 1e4, q["cell_total_i64"], None, 3, 1, return_sums=True)
     finally:
         B.rsc_set_option("grid_ctas", 0)
-    # per-CTA partial sums are added to the global doubles in a different order / split, so
-    # the totals agree to the last bits but need not be identical across grids
-    np.testing.assert_allclose(U.np_(out1["sums"]), U.np_(out2["sums"]), rtol=1e-14)
+    # on-chip sums and the global totals are integers: the sums do not depend on the grid, the
+    # CTA schedule or the order of the atomic adds -- bit-identical
+    assert np.array_equal(U.np_(out1["sums"]), U.np_(out2["sums"]))
     X3 = U.to_dev(indptr, indices, data, 4099)
     out3 = B.rsc_normalize_log1p_moments(X3, 1e4, q["cell_total_i64"], q["gene_n_cells"], 3, 1, return_sums=True)
-    np.testing.assert_allclose(U.np_(out1["sums"]), U.np_(out3["sums"]), rtol=1e-14)
+    assert np.array_equal(U.np_(out1["sums"]), U.np_(out3["sums"]))
+    for k in ("mean_log", "var_log", "mean_lin", "var_lin"):
+        assert torch.equal(out1[k], out2[k]) and torch.equal(out1[k], out3[k]), k
 
 
 def test_fixed_point_extreme_ranges():
