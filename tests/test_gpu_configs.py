@@ -120,6 +120,25 @@ def _sampled_check(cfg, n_cells=None, n_row_samples=384, n_gene_samples=64):
     g = dict(mean_t=out["hvg_mean_t"], disp=out["hvg_disp"], disp_norm=out["hvg_disp_norm"],
              bin=out["hvg_bin"], mask=out["hvg_mask"], indices=out["hvg_indices"], count=out["hvg_count"])
     U.assert_hvg_matches(g, h, cfg.n_top, f"{cfg.name} hvg", strict=False)
+
+    # bench.py's launch configuration: the three staged C-ABI calls with the log-scale set only.
+    # The integer sums make the moments independent of the gene grouping: bit-identical to the
+    # both-sets run above, and so is x''.
+    from paper_2603_02402_b200 import Preprocessor
+    xl_both = X.data.clone()
+    mean_log, var_log = out["mean_log"].clone(), out["var_log"].clone()
+    X.data.copy_(raw)
+    pp1 = Preprocessor(X.n_rows, X.n_cols, X.nnz, cfg.target_sum, cfg.n_top, cfg.n_bins, 1, 1, False)
+    o1 = pp1.run_staged(X, flags)
+    torch.cuda.synchronize()
+    assert torch.equal(X.data, xl_both), "x'' differs between which_moments = 1 and 3"
+    assert torch.equal(o1["mean_log"], mean_log) and torch.equal(o1["var_log"], var_log)
+    for k in ("cell_total_i64", "cell_n_genes", "gene_n_cells", "gene_total_i64"):
+        assert torch.equal(o1[k], out[k]), k
+    hl = O.hvg_select(U.np_(o1["mean_log"]), U.np_(o1["var_log"]), cfg.n_top, cfg.n_bins)
+    gl = dict(mean_t=o1["hvg_mean_t"], disp=o1["hvg_disp"], disp_norm=o1["hvg_disp_norm"],
+              bin=o1["hvg_bin"], mask=o1["hvg_mask"], indices=o1["hvg_indices"], count=o1["hvg_count"])
+    U.assert_hvg_matches(gl, hl, cfg.n_top, f"{cfg.name} hvg on log-scale moments", strict=False)
     return nnz
 
 
