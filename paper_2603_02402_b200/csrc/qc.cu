@@ -23,7 +23,7 @@ namespace rsc {
 constexpr int kQcThreads = 1024;
 constexpr int kQcWarps = kQcThreads / 32;
 #ifndef RSC_QC_RG
-#define RSC_QC_RG 4
+#define RSC_QC_RG 2
 #endif
 constexpr int kQcRowsPerGrab = RSC_QC_RG;
 #ifndef RSC_QC_AHEAD
