@@ -23,6 +23,9 @@ Pins (tests/test_oracle_*.py, `-m "not gpu"`):
   hvg_select       H3/H4 against pandas.cut; per-bin z mean 0 / sd 1; single-gene
                    bin => z == 1; brute-force loops on tiny inputs; hand-worked
                    fixture tests/golden/hvg_tiny.txt.
+  filter_masks     thresholds written out; special cases (no threshold => keep all)
+  subset_csr       dense brute force X[rows][:, cols], scipy.sparse fancy indexing,
+                   identity / drop-all cases, nnz bookkeeping
   The CONSTANTS of H1/H5 (1e-12 floor, 0.1 % edge extension, ddof = 1 inside
   bins, z = 1 rule) are not in PAPER.md ("follows scanpy", L87) and scanpy is
   not installed: those constants are **parity unpinned** against the paper.
@@ -286,3 +289,50 @@ def preprocess_chain(indptr, indices, data, n_genes, gene_flags, target_sum, n_t
         hv = hvg_select(mean_log, var_log, n_top, n_bins)
     return dict(qc=qc, x_norm=xn, x_log=xl, mean_log=mean_log, var_log=var_log,
                 mean_lin=mean_lin, var_lin=var_lin, hvg=hv)
+
+
+# --------------------------------------------------------------------------- NEXT-1: filtering
+def filter_masks(qc: dict, min_genes: int = 0, min_counts: int = 0, max_pct_flag: float = np.inf,
+                 min_cells: int = 0, min_gene_counts: int = 0):
+    """Cell and gene keep-masks from the QC outputs ("filtering"; the
+    thresholds are scanpy's filter_cells / filter_genes arguments, named in SURVEY.md §8(f)
+    NEXT-1; the paper states none).  A cell is kept when it has >= min_genes detected genes,
+    >= min_counts total counts and <= max_pct_flag percent of its counts in the flagged set
+    (a NaN percentage -- an empty cell -- fails any finite max_pct_flag); a gene is kept when
+    it is detected in >= min_cells cells and has >= min_gene_counts total counts."""
+    pct = np.asarray(qc["cell_flag_pct"], F64)
+    cell = (np.asarray(qc["cell_n_genes"], I64) >= min_genes) & \
+           (np.asarray(qc["cell_total_i64"], I64) >= min_counts)
+    if np.isfinite(max_pct_flag):
+        cell &= pct <= max_pct_flag                     # NaN <= x is False
+    gene = (np.asarray(qc["gene_n_cells"], I64) >= min_cells) & \
+           (np.asarray(qc["gene_total_i64"], I64) >= min_gene_counts)
+    return cell.astype(np.uint8), gene.astype(np.uint8)
+
+
+def subset_csr(indptr, indices, data, n_genes: int, keep_rows, keep_cols):
+    """X[keep_rows][:, keep_cols] as a new CSR (filter_cells /
+    filter_genes / HVG column subsetting = row and column removal with a rebuilt int64
+    indptr).  Kept columns are renumbered in ascending order (new index = number of kept
+    columns before it); the stored entries of a kept row keep their order and values; explicit
+    zeros stay stored.  Plain loop over the rows."""
+    indptr = np.asarray(indptr, I64)
+    indices = np.asarray(indices, I32)
+    data = np.asarray(data, F32)
+    keep_rows = np.asarray(keep_rows).astype(bool)
+    keep_cols = np.asarray(keep_cols).astype(bool)
+    assert keep_rows.shape == (len(indptr) - 1,) and keep_cols.shape == (n_genes,)
+    col_map = np.full(n_genes, -1, dtype=I64)
+    col_map[keep_cols] = np.arange(int(keep_cols.sum()), dtype=I64)
+    out_ptr = [0]
+    out_idx, out_val = [], []
+    for i in np.nonzero(keep_rows)[0]:
+        lo, hi = int(indptr[i]), int(indptr[i + 1])
+        j = col_map[indices[lo:hi]]
+        sel = j >= 0
+        out_idx.append(j[sel].astype(I32))
+        out_val.append(data[lo:hi][sel])
+        out_ptr.append(out_ptr[-1] + int(sel.sum()))
+    idx = np.concatenate(out_idx) if out_idx else np.zeros(0, I32)
+    val = np.concatenate(out_val) if out_val else np.zeros(0, F32)
+    return np.asarray(out_ptr, I64), idx.astype(I32), val.astype(F32), int(keep_cols.sum())
