@@ -204,6 +204,44 @@ int rsc_moments_finalize(int32_t n_genes, int64_t n_rows_total, int ddof, const 
                          const double* S2, double* gene_mean, double* gene_var, void* stream);
 
 /* ---------------------------------------------------------------------------------
+ * filtering and subsetting ("filtering"; the
+ * workflow's filter_cells / filter_genes / HVG column subsetting steps, L47).
+ *
+ * rsc_filter_masks: uint8 keep-masks from the QC outputs.  A cell is kept when
+ *   cell_n_genes >= min_genes, cell_total_i64 >= min_counts and cell_flag_pct <= max_pct_flag
+ *   (a NaN percentage fails; max_pct_flag = +inf switches the test off); a gene is kept when
+ *   gene_n_cells >= min_cells and gene_total_i64 >= min_gene_counts.  A NULL input array
+ *   switches its test off; a NULL output mask is not computed.
+ *
+ * rsc_subset_csr_plan / rsc_subset_csr_fill: X[keep_rows][:, keep_cols] as a new CSR.  Kept
+ *   columns are renumbered in ascending order; kept entries keep their order and values
+ *   (explicit zeros stay stored); NULL mask = keep all.  plan writes out_indptr (capacity
+ *   n_rows + 1, the first out_counts[0] + 1 entries are valid) and out_counts = {kept rows,
+ *   kept columns, kept entries} (device int64[3]); the caller reads out_counts (its one
+ *   synchronisation), allocates out_indices / out_data of out_counts[2] elements and calls
+ *   fill with the SAME workspace (it holds the column map and the row offsets).
+ * ------------------------------------------------------------------------------- */
+typedef struct {
+  int32_t min_genes;        /* cells: detected genes              */
+  int32_t min_cells;        /* genes: cells detected in           */
+  int64_t min_counts;       /* cells: total counts                */
+  int64_t min_gene_counts;  /* genes: total counts                */
+  float max_pct_flag;       /* cells: percent in the flagged set; +inf = off */
+  int32_t pad;
+} rsc_filter_params;
+int rsc_filter_masks(int64_t n_rows, int32_t n_cols, const int32_t* cell_n_genes,
+                     const int64_t* cell_total_i64, const float* cell_flag_pct,
+                     const int32_t* gene_n_cells, const int64_t* gene_total_i64,
+                     const rsc_filter_params* prm, uint8_t* cell_keep, uint8_t* gene_keep,
+                     void* stream);
+size_t rsc_subset_csr_workspace_bytes(int64_t n_rows, int32_t n_cols);
+int rsc_subset_csr_plan(const rsc_csr* X, const uint8_t* keep_rows, const uint8_t* keep_cols,
+                        int64_t* out_indptr, int64_t* out_counts, void* ws, size_t ws_bytes,
+                        void* stream);
+int rsc_subset_csr_fill(const rsc_csr* X, const uint8_t* keep_rows, int32_t* out_indices,
+                        float* out_data, void* ws, size_t ws_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------
  * rsc_hvg_select — Seurat-flavour highly-variable-gene selection on the device
  * ("based on per-gene mean and variance"; L39 "gene selection" kernel
  * that avoids CPU<->GPU transfers; L87 "follow the algorithmic implementations of

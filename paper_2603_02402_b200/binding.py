@@ -39,6 +39,7 @@ EXPORTS = [
     "rsc_normalize_log1p_moments_workspace_bytes", "rsc_normalize_log1p_moments",
     "rsc_moments_finalize",
     "rsc_hvg_select_workspace_bytes", "rsc_hvg_select",
+    "rsc_filter_masks", "rsc_subset_csr_workspace_bytes", "rsc_subset_csr_plan", "rsc_subset_csr_fill",
     "rsc_preprocess_workspace_bytes", "rsc_preprocess",
     "rsc_preprocess_host_workspace_bytes", "rsc_preprocess_host",
 ]
@@ -64,6 +65,11 @@ _OUT_FIELDS = ["cell_total_i64", "cell_total_f32", "cell_n_genes", "cell_flag_to
 
 class rsc_outputs(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in _OUT_FIELDS]
+
+
+class rsc_filter_params(C.Structure):
+    _fields_ = [("min_genes", C.c_int32), ("min_cells", C.c_int32), ("min_counts", C.c_int64),
+                ("min_gene_counts", C.c_int64), ("max_pct_flag", C.c_float), ("pad", C.c_int32)]
 
 
 class rsc_params(C.Structure):
@@ -99,6 +105,10 @@ def lib() -> C.CDLL:
     L.rsc_gene_moments_workspace_bytes.argtypes = [i64, i32, i64]
     L.rsc_normalize_log1p_moments_workspace_bytes.argtypes = [i64, i32, i64]
     L.rsc_hvg_select_workspace_bytes.argtypes = [i32, i32]
+    L.rsc_subset_csr_workspace_bytes.argtypes = [i64, i32]
+    L.rsc_filter_masks.argtypes = [i64, i32, p, p, p, p, p, p, p, p, p]
+    L.rsc_subset_csr_plan.argtypes = [p, p, p, p, p, p, sz, p]
+    L.rsc_subset_csr_fill.argtypes = [p, p, p, p, p, sz, p]
     L.rsc_preprocess_workspace_bytes.argtypes = [i64, i32, i64, i32]
     L.rsc_preprocess_host_workspace_bytes.argtypes = [i64, i32, i64, i32]
     L.rsc_set_option.argtypes = [C.c_char_p, C.c_longlong]
@@ -461,3 +471,42 @@ class HostPreprocessor:
                                          C.byref(self.out_struct), _ptr(self.data_out),
                                          _ptr(self.ws), self.ws.numel(), _stream(stream)))
         return self.out
+
+
+# --------------------------------------------------------------------------- NEXT-1: filtering
+def rsc_filter_masks(qc: dict, min_genes: int = 0, min_counts: int = 0,
+                     max_pct_flag: float = float("inf"), min_cells: int = 0,
+                     min_gene_counts: int = 0, stream=None):
+    """uint8 keep-masks (cells, genes) from the outputs of rsc_qc_metrics."""
+    n, G = qc["cell_n_genes"].numel(), qc["gene_n_cells"].numel()
+    dev = qc["cell_n_genes"].device
+    if dev.type != "cuda":
+        raise RscError(RSC_ERR_INVALID_ARG, "rsc_filter_masks needs device tensors (no CPU fallback)")
+    prm = rsc_filter_params(min_genes, min_cells, min_counts, min_gene_counts, max_pct_flag, 0)
+    ck = torch.empty(n, dtype=torch.uint8, device=dev)
+    gk = torch.empty(G, dtype=torch.uint8, device=dev)
+    _check(lib().rsc_filter_masks(n, G, _ptr(qc["cell_n_genes"]), _ptr(qc["cell_total_i64"]),
+                                  _ptr(qc["cell_flag_pct"]), _ptr(qc["gene_n_cells"]),
+                                  _ptr(qc["gene_total_i64"]), C.byref(prm), _ptr(ck), _ptr(gk),
+                                  _stream(stream)))
+    return ck, gk
+
+
+def rsc_subset_csr(X: Csr, keep_rows: Optional[torch.Tensor] = None,
+                   keep_cols: Optional[torch.Tensor] = None, stream=None) -> Csr:
+    """X[keep_rows][:, keep_cols] (uint8 masks or None) as a new device Csr: plan, one read of
+    the three output sizes (the only synchronisation), allocation, fill."""
+    _need_cuda(X)
+    L, dev = lib(), X.device
+    ws = _ws(L.rsc_subset_csr_workspace_bytes(X.n_rows, X.n_cols), dev)
+    out_indptr = torch.empty(X.n_rows + 1, dtype=torch.int64, device=dev)
+    counts = torch.zeros(3, dtype=torch.int64, device=dev)
+    cs = X.c_struct()
+    _check(L.rsc_subset_csr_plan(C.byref(cs), _ptr(keep_rows), _ptr(keep_cols), _ptr(out_indptr),
+                                 _ptr(counts), _ptr(ws), ws.numel(), _stream(stream)))
+    n_out, g_out, nnz_out = (int(v) for v in counts.tolist())
+    out_indices = torch.empty(nnz_out, dtype=torch.int32, device=dev)
+    out_data = torch.empty(nnz_out, dtype=torch.float32, device=dev)
+    _check(L.rsc_subset_csr_fill(C.byref(cs), _ptr(keep_rows), _ptr(out_indices), _ptr(out_data),
+                                 _ptr(ws), ws.numel(), _stream(stream)))
+    return Csr(out_indptr[: n_out + 1], out_indices, out_data, max(g_out, 1), X.sorted_indices), g_out

@@ -252,6 +252,46 @@ size_t rsc_hvg_select_workspace_bytes(int32_t G, int32_t n_bins) {
   return hvg_workspace_bytes(G, n_bins);
 }
 
+int rsc_filter_masks(int64_t n_rows, int32_t n_cols, const int32_t* cell_n_genes,
+                     const int64_t* cell_total_i64, const float* cell_flag_pct,
+                     const int32_t* gene_n_cells, const int64_t* gene_total_i64,
+                     const rsc_filter_params* prm, uint8_t* cell_keep, uint8_t* gene_keep, void* stream) {
+  RSC_CHECK_ARG(prm != nullptr, "rsc_filter_masks: params is NULL");
+  RSC_CHECK_ARG(n_rows >= 0 && n_cols >= 0, "rsc_filter_masks: negative size");
+  RSC_CHECK_ARG(!(prm->max_pct_flag != prm->max_pct_flag), "rsc_filter_masks: max_pct_flag is NaN");
+  int rc = check_device();
+  if (rc) return rc;
+  return launch_filter_masks(n_rows, n_cols, cell_n_genes, cell_total_i64, cell_flag_pct, gene_n_cells,
+                             gene_total_i64, *prm, cell_keep, gene_keep, static_cast<cudaStream_t>(stream));
+}
+
+size_t rsc_subset_csr_workspace_bytes(int64_t n_rows, int32_t n_cols) {
+  return subset_workspace_bytes(n_rows, n_cols);
+}
+
+int rsc_subset_csr_plan(const rsc_csr* X, const uint8_t* keep_rows, const uint8_t* keep_cols,
+                        int64_t* out_indptr, int64_t* out_counts, void* ws, size_t ws_bytes,
+                        void* stream) {
+  int rc = check_csr(X, "rsc_subset_csr_plan", false);
+  if (rc) return rc;
+  RSC_CHECK_ARG(out_indptr != nullptr && out_counts != nullptr, "rsc_subset_csr_plan: output is NULL");
+  if ((rc = check_device())) return rc;
+  if ((rc = check_ws("rsc_subset_csr_plan", ws, ws_bytes, subset_workspace_bytes(X->n_rows, X->n_cols))))
+    return rc;
+  return launch_subset_plan(*X, keep_rows, keep_cols, out_indptr, out_counts, ws,
+                            static_cast<cudaStream_t>(stream));
+}
+
+int rsc_subset_csr_fill(const rsc_csr* X, const uint8_t* keep_rows, int32_t* out_indices,
+                        float* out_data, void* ws, size_t ws_bytes, void* stream) {
+  int rc = check_csr(X, "rsc_subset_csr_fill", true);
+  if (rc) return rc;
+  if ((rc = check_device())) return rc;
+  if ((rc = check_ws("rsc_subset_csr_fill", ws, ws_bytes, subset_workspace_bytes(X->n_rows, X->n_cols))))
+    return rc;
+  return launch_subset_fill(*X, keep_rows, out_indices, out_data, ws, static_cast<cudaStream_t>(stream));
+}
+
 int rsc_hvg_select(int32_t n_genes, const double* gene_mean, const double* gene_var, int32_t n_top,
                    int32_t n_bins, int flags, double* out_mean_t, double* out_disp,
                    double* out_disp_norm, int32_t* out_bin, uint8_t* out_mask,

@@ -100,6 +100,16 @@ int launch_hvg(int32_t G, const double* mean, const double* var, int32_t n_top, 
                void* ws, size_t ws_bytes, cudaStream_t st);
 size_t hvg_workspace_bytes(int32_t G, int32_t n_bins);
 
+int launch_filter_masks(int64_t n_rows, int32_t n_cols, const int32_t* cell_n_genes,
+                        const int64_t* cell_total, const float* cell_pct, const int32_t* gene_n_cells,
+                        const int64_t* gene_total, const rsc_filter_params& p, uint8_t* cell_keep,
+                        uint8_t* gene_keep, cudaStream_t st);
+size_t subset_workspace_bytes(int64_t n_rows, int32_t n_cols);
+int launch_subset_plan(const rsc_csr& X, const uint8_t* keep_rows, const uint8_t* keep_cols,
+                       int64_t* out_indptr, int64_t* out_counts, void* ws, cudaStream_t st);
+int launch_subset_fill(const rsc_csr& X, const uint8_t* keep_rows, int32_t* out_indices, float* out_data,
+                       void* ws, cudaStream_t st);
+
 // ---- device helpers ----------------------------------------------------------------
 #ifdef __CUDACC__
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }

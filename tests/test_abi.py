@@ -42,6 +42,7 @@ def test_struct_layout_matches_header(lib):
     assert B.rsc_csr.indptr.offset == 24 and B.rsc_csr.data.offset == 40
     assert ctypes.sizeof(B.rsc_outputs) == 18 * 8
     assert ctypes.sizeof(B.rsc_params) == 28
+    assert ctypes.sizeof(B.rsc_filter_params) == 32 and B.rsc_filter_params.max_pct_flag.offset == 24
 
 
 def test_workspace_queries(lib):
