@@ -252,6 +252,32 @@ def main():
                                                "chain_nnz_per_s": nnz / (sum(tc) / len(tc) / 1e3)}
             del vp
 
+    # ---- SURVEY 8(f) NEXT-1 on the same matrix: QC-threshold filter + HVG column subsetting
+    next1 = None
+    if not args.no_variants and world == 1:
+        data.copy_(pristine)
+        q = binding.rsc_qc_metrics(X, flags)
+        out_h = pp.run_staged(X, flags, None)              # leaves the HVG mask of the headline run
+        data.copy_(pristine)
+        legs = {"filter (min_genes=200, min_cells=3)": binding.rsc_filter_masks(q, min_genes=200, min_cells=3),
+                "hvg columns": (None, out_h["hvg_mask"])}
+        next1 = {}
+        for name, (ck, gk) in legs.items():
+            ts, Y = [], None
+            for k in range(6):
+                del Y
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); Y, g2 = binding.rsc_subset_csr(X, ck, gk); b.record()
+                torch.cuda.synchronize()
+                if k >= 2:
+                    ts.append(a.elapsed_time(b))
+            ms = sum(ts) / len(ts)
+            byt = 4.0 * nnz + 8.0 * nnz + 8.0 * Y.nnz       # plan reads indices; fill reads both, writes kept
+            next1[name] = {"ms": ms, "nnz_out": Y.nnz, "n_rows_out": Y.n_rows, "n_cols_out": g2,
+                           "GBps": byt / (ms / 1e3) / 1e9,
+                           "note": "plan + size read-back + allocation + fill, CUDA events"}
+        del Y, q
+
     # ---- end to end through the host entry point (rank-local; N=1 only)
     e2e = None
     if not args.no_e2e and world == 1:
@@ -319,7 +345,7 @@ def main():
                    "l2": "inputs (>= 8 B/nnz) larger than L2; data restored from a pristine copy "
                          "between steps (untimed)",
                    "parallelism": "1 GPU" if world == 1 else f"row-sharded x{world} + all-reduce of per-gene sums"},
-        "roofline": roofline, "stages": stages, "variants": variants, "cpu_baseline": cpu, "e2e": e2e,
+        "roofline": roofline, "stages": stages, "variants": variants, "next1_filter_subset": next1, "cpu_baseline": cpu, "e2e": e2e,
         "gpu_launches": int(launches), "clocks": sampler.summary(),
     }
     print(json.dumps(line))
