@@ -41,7 +41,7 @@
 namespace rsc {
 
 #ifndef RSC_FU_THREADS
-#define RSC_FU_THREADS 768
+#define RSC_FU_THREADS 736
 #endif
 constexpr int kFuThreads = RSC_FU_THREADS;
 #ifndef RSC_FU_RG
