@@ -257,26 +257,8 @@ __device__ __forceinline__ uint32_t add_carry_of(uint32_t w, uint32_t o, uint32_
 // entries are in flight together (their slots are distinct: one row, four columns)
 __device__ __forceinline__ void acc_quad(uint32_t base, const uint32_t (&so)[4], const uint32_t (&a)[4]) {
   uint32_t sa[4], o[4], o0[4], q0[4], q1[4];
-#if defined(RSC_EXP) && RSC_EXP == 2
-  return;
-#endif
-#if defined(RSC_EXP) && RSC_EXP == 3
-#pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    sa[k] = base + so[k];
-    unsigned long long q;
-    asm("mul.wide.u32 %0, %1, %1;" : "=l"(q) : "r"(a[k]));
-    reds_add(sa[k], a[k]); reds_add(sa[k] + 8, (uint32_t)q); reds_add(sa[k] + 12, (uint32_t)(q >> 32));
-  }
-  return;
-#endif
 #pragma unroll
   for (int k = 0; k < 4; ++k) { sa[k] = base + so[k]; o[k] = atoms_add(sa[k], a[k]); }
-#if defined(RSC_EXP) && RSC_EXP == 1
-#pragma unroll
-  for (int k = 0; k < 4; ++k) reds_inc_if(sa[k] + 4, carry_of(o[k], a[k]) != 0u);
-  return;
-#endif
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
     unsigned long long q;

@@ -439,7 +439,6 @@ hvg_kernel(int G, const double* __restrict__ mean, const double* __restrict__ va
     }
     __syncthreads();
     if (warp == 0) {                                      // exclusive scan of rcnt in (round, warp) order
-      const int n = rounds * kHvgWarps;
       const int per = rounds;                             // n / 32 entries per lane, contiguous
       int tot = 0;
       for (int i = 0; i < per; ++i) tot += rcnt[lane * per + i];
@@ -456,7 +455,6 @@ hvg_kernel(int G, const double* __restrict__ mean, const double* __restrict__ va
         run += c;
       }
       if (lane == 31) { *out_count = incl; }
-      (void)n;
     }
     __syncthreads();
     if (out_idx != nullptr) {

@@ -20,7 +20,10 @@
 
 namespace rsc {
 
-constexpr int kQcThreads = 1024;
+#ifndef RSC_QC_THREADS
+#define RSC_QC_THREADS 1024
+#endif
+constexpr int kQcThreads = RSC_QC_THREADS;
 constexpr int kQcWarps = kQcThreads / 32;
 #ifndef RSC_QC_RG
 #define RSC_QC_RG 2
