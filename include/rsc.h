@@ -170,7 +170,9 @@ int rsc_gene_moments(const rsc_csr* X, int transform, int ddof,
  *   shared-memory accumulators instead (any value range, slower).
  *   X->indices and X->data must be 16-byte aligned for the streaming kernel (else the generic
  *   kernel serves the call: same results).
- *   row_splits: optional row split table of X (from rsc_qc_metrics / rsc_row_splits);
+ *   row_splits: optional row split table of X (from rsc_qc_metrics / rsc_row_splits; a partial
+ *   table from rsc_qc_metrics_splits must hold the entries rsc_moments_split_blocks lists for
+ *   THIS n_cols and which_moments -- other entries are not read);
  *   NULL -> computed into the workspace when needed.
  *   cell_total_i64 is required (from rsc_qc_metrics).
  *   gene_n_cells: optional hint (from rsc_qc_metrics) used to balance the gene

@@ -120,7 +120,13 @@ subset_count_kernel(int64_t n_rows, const int64_t* __restrict__ indptr, const in
     unsigned c = 0;
     if (keep_rows == nullptr || keep_rows[row] != 0) {
       const int64_t beg = indptr[row], end = indptr[row + 1];
-      for (int64_t p = beg + lane; p < end; p += 32) c += col_map[__ldg(indices + p)] >= 0 ? 1u : 0u;
+      for (int64_t p0 = beg; p0 < end; p0 += 128) {       // 4 independent loads per lane in flight
+        int j[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { const int64_t p = p0 + u * 32 + lane; j[u] = p < end ? __ldg(indices + p) : -1; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) c += (j[u] >= 0 && col_map[j[u]] >= 0) ? 1u : 0u;
+      }
     }
     c = warp_sum(c);
     if (lane == 0) row_cnt[row] = c;
@@ -217,18 +223,26 @@ subset_fill_kernel(int64_t n_rows, const int64_t* __restrict__ indptr, const int
     if (keep_rows != nullptr && keep_rows[row] == 0) continue;
     const int64_t beg = indptr[row], end = indptr[row + 1];
     int64_t o = row_off[row];
-    for (int64_t p0 = beg; p0 < end; p0 += 32) {
-      const int64_t p = p0 + lane;
-      int j = -1;
-      float x = 0.0f;
-      if (p < end) { j = col_map[__ldg(indices + p)]; x = data[p]; }
-      const unsigned bal = __ballot_sync(0xffffffffu, j >= 0);
-      if (j >= 0) {
-        const int64_t q = o + __popc(bal & ((1u << lane) - 1u));
-        out_indices[q] = j;
-        out_data[q] = x;
+    for (int64_t p0 = beg; p0 < end; p0 += 128) {         // 4 independent loads per lane in flight
+      int j[4];
+      float x[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int64_t p = p0 + u * 32 + lane;
+        j[u] = p < end ? __ldg(indices + p) : -1;
+        x[u] = p < end ? __ldg(data + p) : 0.0f;
       }
-      o += __popc(bal);
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int jn = j[u] >= 0 ? col_map[j[u]] : -1;
+        const unsigned bal = __ballot_sync(0xffffffffu, jn >= 0);
+        if (jn >= 0) {
+          const int64_t q = o + __popc(bal & ((1u << lane) - 1u));
+          out_indices[q] = jn;
+          out_data[q] = x[u];
+        }
+        o += __popc(bal);
+      }
     }
   }
 }
