@@ -56,8 +56,46 @@ __host__ __device__ inline HvgSmem hvg_smem(int G, int n_bins) {
   return m;
 }
 
+// H1 / H2 on many CTAs (two fp64 logarithms per gene are the one compute-heavy part): dispersion
+// and transforms of one gene per thread, min / max of the transformed mean per block
+constexpr int kHvgTBlock = 256;
+__global__ void __launch_bounds__(kHvgTBlock)
+hvg_transform_kernel(int G, const double* __restrict__ mean, const double* __restrict__ var, int flags,
+                     double* __restrict__ m_arr, double* __restrict__ d_arr, double* __restrict__ blk_mm) {
+  __shared__ double s_lo[kHvgTBlock / 32], s_hi[kHvgTBlock / 32];
+  const int g = blockIdx.x * kHvgTBlock + threadIdx.x;
+  const double kNaN = __longlong_as_double(0x7ff8000000000000ll);
+  double lo = __longlong_as_double(0x7ff0000000000000ll), hi = -lo;
+  if (g < G) {
+    double mu = mean[g];
+    if (mu == 0.0) mu = 1e-12;
+    double d = __ddiv_rn(var[g], mu);
+    double m = mu;
+    if (flags & RSC_HVG_SEURAT_LOG) {
+      if (d == 0.0) d = kNaN;
+      d = log(d);
+      m = log1p(mu);
+    }
+    m_arr[g] = m;
+    d_arr[g] = d;
+    lo = m; hi = m;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+    hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+  }
+  if ((threadIdx.x & 31) == 0) { s_lo[threadIdx.x >> 5] = lo; s_hi[threadIdx.x >> 5] = hi; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < kHvgTBlock / 32; ++w) { lo = fmin(lo, s_lo[w]); hi = fmax(hi, s_hi[w]); }
+    blk_mm[2 * blockIdx.x] = lo;
+    blk_mm[2 * blockIdx.x + 1] = hi;
+  }
+}
+
 __global__ void __launch_bounds__(kHvgThreads)
-hvg_kernel(int G, const double* __restrict__ mean, const double* __restrict__ var, int n_top,
+hvg_kernel(int G, const double* __restrict__ blk_mm, int n_tblocks, int n_top,
            int n_bins, int flags, double* __restrict__ m_arr, double* __restrict__ d_arr,
            double* __restrict__ z_arr, int32_t* __restrict__ bin_arr,
            uint8_t* __restrict__ out_mask, int32_t* __restrict__ out_idx,
@@ -81,34 +119,11 @@ hvg_kernel(int G, const double* __restrict__ mean, const double* __restrict__ va
   const double kNaN = __longlong_as_double(0x7ff8000000000000ll);
   constexpr int kStride = kHvgBatch * kHvgThreads;
 
-  // H1 / H2: dispersion and transforms; min / max of the transformed mean
+  // H1 / H2 were done by hvg_transform_kernel; min / max of the transformed mean over its blocks
   double lo = __longlong_as_double(0x7ff0000000000000ll), hi = -lo;
-  for (int g0 = tid; g0 < G; g0 += kStride) {
-    double mu8[kHvgBatch], vv8[kHvgBatch];
-#pragma unroll
-    for (int u = 0; u < kHvgBatch; ++u) {
-      const int g = g0 + u * kHvgThreads;
-      mu8[u] = g < G ? mean[g] : 1.0;
-      vv8[u] = g < G ? var[g] : 1.0;
-    }
-#pragma unroll 2
-    for (int u = 0; u < kHvgBatch; ++u) {
-      const int g = g0 + u * kHvgThreads;
-      if (g >= G) break;
-      double mu = mu8[u];
-      if (mu == 0.0) mu = 1e-12;
-      double d = __ddiv_rn(vv8[u], mu);
-      double m = mu;
-      if (flags & RSC_HVG_SEURAT_LOG) {
-        if (d == 0.0) d = kNaN;
-        d = log(d);
-        m = log1p(mu);
-      }
-      m_arr[g] = m;
-      d_arr[g] = d;
-      lo = fmin(lo, m);
-      hi = fmax(hi, m);
-    }
+  for (int i = tid; i < n_tblocks; i += kHvgThreads) {
+    lo = fmin(lo, blk_mm[2 * i]);
+    hi = fmax(hi, blk_mm[2 * i + 1]);
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -494,7 +509,9 @@ hvg_kernel(int G, const double* __restrict__ mean, const double* __restrict__ va
 
 size_t hvg_workspace_bytes(int32_t G, int32_t /*n_bins*/) {
   // m, d, z (double) + bin (int32), each 256-byte aligned
-  return 3 * align_up(sizeof(double) * (size_t)G, 256) + align_up(sizeof(int32_t) * (size_t)G, 256);
+  const size_t tb = ((size_t)G + kHvgTBlock - 1) / kHvgTBlock;
+  return 3 * align_up(sizeof(double) * (size_t)G, 256) + align_up(sizeof(int32_t) * (size_t)G, 256) +
+         align_up(sizeof(double) * 2 * tb, 256);
 }
 
 int launch_hvg(int32_t G, const double* mean, const double* var, int32_t n_top, int32_t n_bins,
@@ -518,7 +535,11 @@ int launch_hvg(int32_t G, const double* mean, const double* var, int32_t n_top, 
     RSC_CUDA(cudaFuncSetAttribute(hvg_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)smem));
   }
-  hvg_kernel<<<1, kHvgThreads, smem, st>>>(G, mean, var, n_top, n_bins, flags, m_arr, d_arr, z_arr,
+  const int tb = (G + kHvgTBlock - 1) / kHvgTBlock;
+  double* blk_mm = reinterpret_cast<double*>(w + 3 * dsz + align_up(sizeof(int32_t) * (size_t)G, 256));
+  hvg_transform_kernel<<<tb, kHvgTBlock, 0, st>>>(G, mean, var, flags, m_arr, d_arr, blk_mm);
+  RSC_LAUNCH_CHECK("hvg_transform_kernel");
+  hvg_kernel<<<1, kHvgThreads, smem, st>>>(G, blk_mm, tb, n_top, n_bins, flags, m_arr, d_arr, z_arr,
                                            b_arr, out_mask, out_indices, out_count);
   RSC_LAUNCH_CHECK("hvg_kernel");
   return RSC_OK;
