@@ -29,8 +29,8 @@ NOMINAL_HBM_GBS = 8000.0          # BASELINE.json's denominator ("fraction of 8 
 FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 BYTES_PER_NNZ = {"qc": 8.0, "fused": 12.0, "chain": 20.0}   # SURVEY.md §8(d), DESIGN.md §7
 # dram__bytes_read.sum + dram__bytes_write.sum of one fused-pass launch, from the ncu --set full
-# capture D in profiles/r01c_cfg3.md; key = (config, which_moments), full-size runs only
-NCU_TRAFFIC_BYTES = {(3, 1): 12.319117e9 + 5.892285e9}
+# capture E in profiles/r01c_cfg3.md; key = (config, which_moments), full-size runs only
+NCU_TRAFFIC_BYTES = {(3, 1): 11.979356e9 + 5.863033e9}
 
 
 def parse_args():
