@@ -26,6 +26,8 @@ Pins (tests/test_oracle_*.py, `-m "not gpu"`):
   filter_masks     thresholds written out; special cases (no threshold => keep all)
   subset_csr       dense brute force X[rows][:, cols], scipy.sparse fancy indexing,
                    identity / drop-all cases, nnz bookkeeping
+  scale_dense      dense (X - mean) / sd with numpy; column mean 0 / sd 1 when unclipped;
+                   zero-variance gene => sd 1; clip bounds; zero_center = False keeps zeros
   The CONSTANTS of H1/H5 (1e-12 floor, 0.1 % edge extension, ddof = 1 inside
   bins, z = 1 rule) are not in PAPER.md ("follows scanpy", L87) and scanpy is
   not installed: those constants are **parity unpinned** against the paper.
@@ -336,3 +338,26 @@ def subset_csr(indptr, indices, data, n_genes: int, keep_rows, keep_cols):
     idx = np.concatenate(out_idx) if out_idx else np.zeros(0, I32)
     val = np.concatenate(out_val) if out_val else np.zeros(0, F32)
     return np.asarray(out_ptr, I64), idx.astype(I32), val.astype(F32), int(keep_cols.sum())
+
+
+# --------------------------------------------------------------------------- NEXT-3 (first half): scale
+def scale_dense(indptr, indices, data, n_genes: int, gene_mean, gene_var, max_value=None,
+                zero_center: bool = True):
+    """z-score per gene, optionally clipped ("scaling"; SURVEY.md §8(f)
+    NEXT-3 "scale: z-score using the log-scale moments already produced").  Dense float32
+    [n_rows, n_genes] output:  y_ij = (x_ij - mean_j) / sd_j  with sd_j = sqrt(var_j) and
+    sd_j = 1 where var_j == 0 (reading R16: scanpy's convention; the paper gives
+    none); zero_center = False divides only (zeros stay zero).  max_value: clip to
+    [-max_value, max_value] when centred, to (-inf, max_value] otherwise (R16)."""
+    indptr = np.asarray(indptr, I64)
+    n = len(indptr) - 1
+    mean = np.asarray(gene_mean, F64)
+    sd = np.sqrt(np.asarray(gene_var, F64))
+    sd = np.where(sd == 0.0, 1.0, sd)
+    dense = np.zeros((n, n_genes), dtype=F64)
+    rows = _row_ids(indptr)
+    dense[rows, np.asarray(indices, I64)] = np.asarray(data, F64)
+    y = (dense - mean[None, :]) / sd[None, :] if zero_center else dense / sd[None, :]
+    if max_value is not None:
+        y = np.clip(y, -max_value if zero_center else -np.inf, max_value)
+    return y.astype(F32)
