@@ -276,6 +276,22 @@ def main():
             next1[name] = {"ms": ms, "nnz_out": Y.nnz, "n_rows_out": Y.n_rows, "n_cols_out": g2,
                            "GBps": byt / (ms / 1e3) / 1e9,
                            "note": "plan + size read-back + allocation + fill, CUDA events"}
+        # NEXT-3 (first half): dense z-scores of the HVG-subset matrix (Y of the last leg)
+        sel = torch.nonzero(out_h["hvg_mask"]).flatten()
+        mu, vv = out_h["mean_log"][sel].contiguous(), out_h["var_log"][sel].contiguous()
+        ts = []
+        for k in range(5):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); Zs = binding.rsc_scale_dense(Y, mu, vv, 10.0, True); b.record()
+            torch.cuda.synchronize()
+            if k >= 2:
+                ts.append(a.elapsed_time(b))
+            del Zs
+        ms = sum(ts) / len(ts)
+        next1["scale (dense, HVG columns, max_value=10)"] = {
+            "ms": ms, "out_elements": Y.n_rows * g2,
+            "GBps": (4.0 * Y.n_rows * g2 + 8.0 * Y.nnz) / (ms / 1e3) / 1e9,
+            "note": "writes n_rows x n_cols float32; reads the subset CSR"}
         del Y, q
 
     # ---- end to end through the host entry point (rank-local; N=1 only)
@@ -345,7 +361,7 @@ def main():
                    "l2": "inputs (>= 8 B/nnz) larger than L2; data restored from a pristine copy "
                          "between steps (untimed)",
                    "parallelism": "1 GPU" if world == 1 else f"row-sharded x{world} + all-reduce of per-gene sums"},
-        "roofline": roofline, "stages": stages, "variants": variants, "next1_filter_subset": next1, "cpu_baseline": cpu, "e2e": e2e,
+        "roofline": roofline, "stages": stages, "variants": variants, "next_filter_subset_scale": next1, "cpu_baseline": cpu, "e2e": e2e,
         "gpu_launches": int(launches), "clocks": sampler.summary(),
     }
     print(json.dumps(line))

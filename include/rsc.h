@@ -244,6 +244,21 @@ int rsc_subset_csr_fill(const rsc_csr* X, const uint8_t* keep_rows, int32_t* out
                         float* out_data, void* ws, size_t ws_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------------
+ * SURVEY.md 8(f) NEXT-3 (first half) -- rsc_scale_dense: z-score per gene with optional clip
+ * ("scaling"), written as a DENSE row-major float32 [n_rows, n_cols] matrix
+ * (run it after subsetting to the HVGs: the output has n_rows * n_cols elements):
+ *     out[i][j] = clip((x_ij - gene_mean[j]) / sd_j),  sd_j = sqrt(gene_var[j]), 1 where it is 0
+ *   zero_center = 0: out = x_ij / sd_j (zeros stay zero).  max_value > 0: clip to
+ *   [-max_value, max_value] (zero_center) or (-inf, max_value]; max_value <= 0: no clip.
+ *   gene_mean / gene_var: e.g. mean_log / var_log of rsc_normalize_log1p_moments (ddof 1).
+ *   ws: rsc_scale_dense_workspace_bytes(n_cols) bytes.  X is not modified.
+ * ------------------------------------------------------------------------------- */
+size_t rsc_scale_dense_workspace_bytes(int32_t n_cols);
+int rsc_scale_dense(const rsc_csr* X, const double* gene_mean, const double* gene_var,
+                    float max_value, int zero_center, float* out, void* ws, size_t ws_bytes,
+                    void* stream);
+
+/* ---------------------------------------------------------------------------------
  * rsc_hvg_select — Seurat-flavour highly-variable-gene selection on the device
  * ("based on per-gene mean and variance"; L39 "gene selection" kernel
  * that avoids CPU<->GPU transfers; L87 "follow the algorithmic implementations of

@@ -40,6 +40,7 @@ EXPORTS = [
     "rsc_moments_finalize",
     "rsc_hvg_select_workspace_bytes", "rsc_hvg_select",
     "rsc_filter_masks", "rsc_subset_csr_workspace_bytes", "rsc_subset_csr_plan", "rsc_subset_csr_fill",
+    "rsc_scale_dense_workspace_bytes", "rsc_scale_dense",
     "rsc_preprocess_workspace_bytes", "rsc_preprocess",
     "rsc_preprocess_host_workspace_bytes", "rsc_preprocess_host",
 ]
@@ -106,6 +107,8 @@ def lib() -> C.CDLL:
     L.rsc_normalize_log1p_moments_workspace_bytes.argtypes = [i64, i32, i64]
     L.rsc_hvg_select_workspace_bytes.argtypes = [i32, i32]
     L.rsc_subset_csr_workspace_bytes.argtypes = [i64, i32]
+    L.rsc_scale_dense_workspace_bytes.argtypes = [i32]
+    L.rsc_scale_dense.argtypes = [p, p, p, flt, C.c_int, p, p, sz, p]
     L.rsc_filter_masks.argtypes = [i64, i32, p, p, p, p, p, p, p, p, p]
     L.rsc_subset_csr_plan.argtypes = [p, p, p, p, p, p, sz, p]
     L.rsc_subset_csr_fill.argtypes = [p, p, p, p, p, sz, p]
@@ -510,3 +513,18 @@ def rsc_subset_csr(X: Csr, keep_rows: Optional[torch.Tensor] = None,
     _check(L.rsc_subset_csr_fill(C.byref(cs), _ptr(keep_rows), _ptr(out_indices), _ptr(out_data),
                                  _ptr(ws), ws.numel(), _stream(stream)))
     return Csr(out_indptr[: n_out + 1], out_indices, out_data, max(g_out, 1), X.sorted_indices), g_out
+
+
+# --------------------------------------------------------------------------- NEXT-3: scale
+def rsc_scale_dense(X: Csr, gene_mean: torch.Tensor, gene_var: torch.Tensor,
+                    max_value: Optional[float] = None, zero_center: bool = True, stream=None) -> torch.Tensor:
+    """Dense float32 [n_rows, n_cols] z-scores (clipped to max_value if given)."""
+    _need_cuda(X)
+    L = lib()
+    out = torch.empty((X.n_rows, X.n_cols), dtype=torch.float32, device=X.device)
+    ws = _ws(L.rsc_scale_dense_workspace_bytes(X.n_cols), X.device)
+    cs = X.c_struct()
+    _check(L.rsc_scale_dense(C.byref(cs), _ptr(gene_mean), _ptr(gene_var),
+                             float(max_value) if max_value is not None else 0.0, int(bool(zero_center)),
+                             _ptr(out), _ptr(ws), ws.numel(), _stream(stream)))
+    return out

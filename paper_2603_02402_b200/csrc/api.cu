@@ -292,6 +292,22 @@ int rsc_subset_csr_fill(const rsc_csr* X, const uint8_t* keep_rows, int32_t* out
   return launch_subset_fill(*X, keep_rows, out_indices, out_data, ws, static_cast<cudaStream_t>(stream));
 }
 
+size_t rsc_scale_dense_workspace_bytes(int32_t n_cols) { return scale_workspace_bytes(n_cols); }
+
+int rsc_scale_dense(const rsc_csr* X, const double* gene_mean, const double* gene_var,
+                    float max_value, int zero_center, float* out, void* ws, size_t ws_bytes,
+                    void* stream) {
+  int rc = check_csr(X, "rsc_scale_dense", true);
+  if (rc) return rc;
+  RSC_CHECK_ARG(gene_mean != nullptr && gene_var != nullptr, "rsc_scale_dense: mean / var is NULL");
+  RSC_CHECK_ARG(out != nullptr || X->n_rows == 0, "rsc_scale_dense: out is NULL");
+  RSC_CHECK_ARG(!(max_value != max_value), "rsc_scale_dense: max_value is NaN");
+  if ((rc = check_device())) return rc;
+  if ((rc = check_ws("rsc_scale_dense", ws, ws_bytes, scale_workspace_bytes(X->n_cols)))) return rc;
+  return launch_scale_dense(*X, gene_mean, gene_var, max_value, zero_center, out, ws,
+                            static_cast<cudaStream_t>(stream));
+}
+
 int rsc_hvg_select(int32_t n_genes, const double* gene_mean, const double* gene_var, int32_t n_top,
                    int32_t n_bins, int flags, double* out_mean_t, double* out_disp,
                    double* out_disp_norm, int32_t* out_bin, uint8_t* out_mask,

@@ -1,0 +1,88 @@
+// SURVEY.md 8(f) NEXT-3 (first half): scale -- z-score per gene with optional clip ("scaling",
+// PAPER.md:L61, L151), from the per-gene mean / variance the preprocessing chain already produced.
+// The output is DENSE float32 [n_rows, n_cols] (the step densifies; it follows HVG subsetting):
+//     y_ij = clip((x_ij - mean_j) / sd_j),  sd_j = sqrt(var_j), 1 where var_j == 0
+// Every row is first filled with the per-gene value of a zero entry (one 128-bit store per lane,
+// from a small table), then the row's stored entries overwrite their positions; the entries are
+// computed in fp64 (no cancellation error near the mean).  Write-bound: 4 B x n_rows x n_cols.
+#include <math.h>
+
+#include "common.cuh"
+
+namespace rsc {
+
+// per-gene sd (double; 1 where the variance is 0) and the value of a zero entry (float, clipped)
+__global__ void __launch_bounds__(256)
+scale_prep_kernel(int32_t G, const double* __restrict__ mean, const double* __restrict__ var,
+                  float max_value, int zero_center, double* __restrict__ sd_out, float* __restrict__ base) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= G) return;
+  double sd = sqrt(var[j]);
+  if (sd == 0.0) sd = 1.0;
+  sd_out[j] = sd;                                          // the entries divide by sd (as the definition)
+  double b = zero_center ? (0.0 - mean[j]) / sd : 0.0;
+  if (max_value > 0.0f) {
+    if (b > (double)max_value) b = (double)max_value;
+    if (zero_center && b < -(double)max_value) b = -(double)max_value;
+  }
+  base[j] = (float)b;
+}
+
+__global__ void __launch_bounds__(256)
+scale_dense_kernel(int64_t n_rows, int32_t G, const int64_t* __restrict__ indptr,
+                   const int32_t* __restrict__ indices, const float* __restrict__ data,
+                   const double* __restrict__ mean, const double* __restrict__ sd,
+                   const float* __restrict__ base, float max_value, int zero_center,
+                   float* __restrict__ out) {
+  const int lane = lane_id();
+  const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  const bool vec = (G & 3) == 0 && ((reinterpret_cast<uintptr_t>(out) | reinterpret_cast<uintptr_t>(base)) & 15) == 0;
+  for (int64_t row = warp0; row < n_rows; row += nwarps) {
+    float* o = out + row * (int64_t)G;
+    if (vec) {
+      for (int j = lane * 4; j < G; j += 128)
+        *reinterpret_cast<float4*>(o + j) = __ldg(reinterpret_cast<const float4*>(base + j));
+    } else {
+      for (int j = lane; j < G; j += 32) o[j] = __ldg(base + j);
+    }
+    __syncwarp();                                          // the fill is ordered before the overwrites
+    const int64_t beg = indptr[row], end = indptr[row + 1];
+    for (int64_t p = beg + lane; p < end; p += 32) {
+      const int j = __ldg(indices + p);
+      double y = (double)__ldg(data + p);
+      if (zero_center) y -= mean[j];
+      y = y / sd[j];
+      if (max_value > 0.0f) {
+        if (y > (double)max_value) y = (double)max_value;
+        if (zero_center && y < -(double)max_value) y = -(double)max_value;
+      }
+      o[j] = (float)y;
+    }
+  }
+}
+
+size_t scale_workspace_bytes(int32_t n_cols) {
+  return align_up(sizeof(double) * (size_t)(n_cols > 0 ? n_cols : 0), 256) +
+         align_up(sizeof(float) * (size_t)(n_cols > 0 ? n_cols : 0), 256);
+}
+
+int launch_scale_dense(const rsc_csr& X, const double* gene_mean, const double* gene_var,
+                       float max_value, int zero_center, float* out, void* ws, cudaStream_t st) {
+  if (X.n_rows == 0) return RSC_OK;
+  unsigned char* w = static_cast<unsigned char*>(ws);
+  double* sd = reinterpret_cast<double*>(w);
+  float* base = reinterpret_cast<float*>(w + align_up(sizeof(double) * (size_t)X.n_cols, 256));
+  scale_prep_kernel<<<(X.n_cols + 255) / 256, 256, 0, st>>>(X.n_cols, gene_mean, gene_var, max_value,
+                                                            zero_center, sd, base);
+  RSC_LAUNCH_CHECK("scale_prep_kernel");
+  int64_t blocks = (X.n_rows + 7) / 8;
+  const int64_t cap = (int64_t)sm_count() * 16;
+  if (blocks > cap) blocks = cap;
+  scale_dense_kernel<<<(unsigned)blocks, 256, 0, st>>>(X.n_rows, X.n_cols, X.indptr, X.indices, X.data,
+                                                       gene_mean, sd, base, max_value, zero_center, out);
+  RSC_LAUNCH_CHECK("scale_dense_kernel");
+  return RSC_OK;
+}
+
+}  // namespace rsc
