@@ -28,6 +28,7 @@ Pins (tests/test_oracle_*.py, `-m "not gpu"`):
                    identity / drop-all cases, nnz bookkeeping
   scale_dense      dense (X - mean) / sd with numpy; column mean 0 / sd 1 when unclipped;
                    zero-variance gene => sd 1; clip bounds; zero_center = False keeps zeros
+  hvg_cutoffs      window tests written out with loops; infinite window == all non-NaN z
   The CONSTANTS of H1/H5 (1e-12 floor, 0.1 % edge extension, ddof = 1 inside
   bins, z = 1 rule) are not in PAPER.md ("follows scanpy", L87) and scanpy is
   not installed: those constants are **parity unpinned** against the paper.
@@ -361,3 +362,17 @@ def scale_dense(indptr, indices, data, n_genes: int, gene_mean, gene_var, max_va
     if max_value is not None:
         y = np.clip(y, -max_value if zero_center else -np.inf, max_value)
     return y.astype(F32)
+
+
+# --------------------------------------------------------------------------- NEXT-4 (part): cutoffs
+def hvg_cutoffs(mean_t, disp_norm, min_mean=0.0125, max_mean=3.0, min_disp=0.5, max_disp=np.inf):
+    """Threshold-based HVG selection (SURVEY.md §8(f) NEXT-4 "threshold-based selection
+    (mean/dispersion windows)"): from the transformed mean m and the normalised dispersion z of
+    hvg_select, gene j is selected when  min_mean < m_j < max_mean  and  min_disp < z_j <
+    max_disp  (strict; a NaN z fails).  The defaults and the strictness are scanpy's (the paper
+    gives none: parity unpinned against PAPER.md, reading R17)."""
+    m = np.asarray(mean_t, F64)
+    z = np.asarray(disp_norm, F64)
+    with np.errstate(invalid="ignore"):
+        mask = (m > min_mean) & (m < max_mean) & (z > min_disp) & (z < max_disp)
+    return dict(mask=mask.astype(np.uint8), indices=np.nonzero(mask)[0].astype(I32), count=int(mask.sum()))

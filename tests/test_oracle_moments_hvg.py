@@ -199,3 +199,17 @@ def test_hvg_edge_cases():
     np.testing.assert_allclose(h1["disp_norm"], h0["disp_norm"][p], rtol=1e-10, equal_nan=True)
     assert np.array_equal(h1["mask"], h0["mask"][p])
     assert h0["count"] == 20
+
+
+def test_hvg_cutoffs_loops_and_special_windows():
+    """NEXT-4 (part): window selection against explicit loops; infinite window == all non-NaN z."""
+    rng = np.random.default_rng(3)
+    m = rng.uniform(0, 4, 500); z = rng.normal(0, 1.5, 500); z[::17] = np.nan
+    o = O.hvg_cutoffs(m, z)
+    want = [j for j in range(500) if 0.0125 < m[j] < 3.0 and z[j] > 0.5 and not np.isnan(z[j])]
+    assert o["indices"].tolist() == want and o["count"] == len(want) and o["mask"].sum() == len(want)
+    o = O.hvg_cutoffs(m, z, -np.inf, np.inf, -np.inf, np.inf)
+    assert o["count"] == int((~np.isnan(z)).sum())
+    assert O.hvg_cutoffs(m, z, 1.0, 1.0)["count"] == 0              # empty (strict) window
+    m2 = np.array([0.0125, 3.0, 1.0]); z2 = np.array([1.0, 1.0, 0.5])
+    assert O.hvg_cutoffs(m2, z2)["count"] == 0                      # every bound is strict
