@@ -244,6 +244,17 @@ int rsc_subset_csr_fill(const rsc_csr* X, const uint8_t* keep_rows, int32_t* out
                         float* out_data, void* ws, size_t ws_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------------
+ * rsc_hvg_cutoffs: threshold-based HVG selection from the
+ * outputs of rsc_hvg_select (out_mean_t = m, out_disp_norm = z): gene j is selected when
+ * min_mean < m_j < max_mean and min_disp < z_j < max_disp (strict; a NaN z fails; use
+ * -inf / +inf to switch a bound off).  out_mask uint8[n_genes] and out_count int32[1] are
+ * required; out_indices int32[n_genes] (selected genes, ascending) is optional.
+ * ------------------------------------------------------------------------------- */
+int rsc_hvg_cutoffs(int32_t n_genes, const double* mean_t, const double* disp_norm,
+                    double min_mean, double max_mean, double min_disp, double max_disp,
+                    uint8_t* out_mask, int32_t* out_indices, int32_t* out_count, void* stream);
+
+/* ---------------------------------------------------------------------------------
  * SURVEY.md 8(f) NEXT-3 (first half) -- rsc_scale_dense: z-score per gene with optional clip
  * ("scaling"), written as a DENSE row-major float32 [n_rows, n_cols] matrix
  * (run it after subsetting to the HVGs: the output has n_rows * n_cols elements):

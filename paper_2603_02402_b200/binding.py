@@ -40,7 +40,7 @@ EXPORTS = [
     "rsc_moments_finalize",
     "rsc_hvg_select_workspace_bytes", "rsc_hvg_select",
     "rsc_filter_masks", "rsc_subset_csr_workspace_bytes", "rsc_subset_csr_plan", "rsc_subset_csr_fill",
-    "rsc_scale_dense_workspace_bytes", "rsc_scale_dense",
+    "rsc_scale_dense_workspace_bytes", "rsc_scale_dense", "rsc_hvg_cutoffs",
     "rsc_preprocess_workspace_bytes", "rsc_preprocess",
     "rsc_preprocess_host_workspace_bytes", "rsc_preprocess_host",
 ]
@@ -108,6 +108,7 @@ def lib() -> C.CDLL:
     L.rsc_hvg_select_workspace_bytes.argtypes = [i32, i32]
     L.rsc_subset_csr_workspace_bytes.argtypes = [i64, i32]
     L.rsc_scale_dense_workspace_bytes.argtypes = [i32]
+    L.rsc_hvg_cutoffs.argtypes = [i32, p, p, C.c_double, C.c_double, C.c_double, C.c_double, p, p, p, p]
     L.rsc_scale_dense.argtypes = [p, p, p, flt, C.c_int, p, p, sz, p]
     L.rsc_filter_masks.argtypes = [i64, i32, p, p, p, p, p, p, p, p, p]
     L.rsc_subset_csr_plan.argtypes = [p, p, p, p, p, p, sz, p]
@@ -527,4 +528,20 @@ def rsc_scale_dense(X: Csr, gene_mean: torch.Tensor, gene_var: torch.Tensor,
     _check(L.rsc_scale_dense(C.byref(cs), _ptr(gene_mean), _ptr(gene_var),
                              float(max_value) if max_value is not None else 0.0, int(bool(zero_center)),
                              _ptr(out), _ptr(ws), ws.numel(), _stream(stream)))
+    return out
+
+
+# --------------------------------------------------------------------------- NEXT-4 (part): cutoffs
+def rsc_hvg_cutoffs(mean_t: torch.Tensor, disp_norm: torch.Tensor, min_mean: float = 0.0125,
+                    max_mean: float = 3.0, min_disp: float = 0.5, max_disp: float = float("inf"),
+                    stream=None) -> dict:
+    """Threshold-based HVG selection from rsc_hvg_select's mean_t / disp_norm outputs."""
+    if mean_t.device.type != "cuda":
+        raise RscError(RSC_ERR_INVALID_ARG, "device tensors required (no CPU fallback)")
+    G, dev = mean_t.numel(), mean_t.device
+    out = dict(mask=torch.empty(G, dtype=torch.uint8, device=dev),
+               indices=torch.empty(G, dtype=torch.int32, device=dev),
+               count=torch.zeros(1, dtype=torch.int32, device=dev))
+    _check(lib().rsc_hvg_cutoffs(G, _ptr(mean_t), _ptr(disp_norm), min_mean, max_mean, min_disp, max_disp,
+                                 _ptr(out["mask"]), _ptr(out["indices"]), _ptr(out["count"]), _stream(stream)))
     return out

@@ -292,6 +292,20 @@ int rsc_subset_csr_fill(const rsc_csr* X, const uint8_t* keep_rows, int32_t* out
   return launch_subset_fill(*X, keep_rows, out_indices, out_data, ws, static_cast<cudaStream_t>(stream));
 }
 
+int rsc_hvg_cutoffs(int32_t n_genes, const double* mean_t, const double* disp_norm,
+                    double min_mean, double max_mean, double min_disp, double max_disp,
+                    uint8_t* out_mask, int32_t* out_indices, int32_t* out_count, void* stream) {
+  RSC_CHECK_ARG(n_genes > 0, "rsc_hvg_cutoffs: n_genes <= 0");
+  RSC_CHECK_ARG(mean_t != nullptr && disp_norm != nullptr, "rsc_hvg_cutoffs: input is NULL");
+  RSC_CHECK_ARG(out_mask != nullptr && out_count != nullptr, "rsc_hvg_cutoffs: out_mask / out_count is NULL");
+  RSC_CHECK_ARG(!(min_mean != min_mean) && !(max_mean != max_mean) && !(min_disp != min_disp) &&
+                !(max_disp != max_disp), "rsc_hvg_cutoffs: a bound is NaN");
+  int rc = check_device();
+  if (rc) return rc;
+  return launch_hvg_cutoffs(n_genes, mean_t, disp_norm, min_mean, max_mean, min_disp, max_disp, out_mask,
+                            out_indices, out_count, static_cast<cudaStream_t>(stream));
+}
+
 size_t rsc_scale_dense_workspace_bytes(int32_t n_cols) { return scale_workspace_bytes(n_cols); }
 
 int rsc_scale_dense(const rsc_csr* X, const double* gene_mean, const double* gene_var,

@@ -110,6 +110,9 @@ int launch_subset_plan(const rsc_csr& X, const uint8_t* keep_rows, const uint8_t
 int launch_subset_fill(const rsc_csr& X, const uint8_t* keep_rows, int32_t* out_indices, float* out_data,
                        void* ws, cudaStream_t st);
 
+int launch_hvg_cutoffs(int32_t G, const double* mean_t, const double* disp_norm, double min_mean,
+                       double max_mean, double min_disp, double max_disp, uint8_t* out_mask,
+                       int32_t* out_idx, int32_t* out_count, cudaStream_t st);
 size_t scale_workspace_bytes(int32_t n_cols);
 int launch_scale_dense(const rsc_csr& X, const double* gene_mean, const double* gene_var,
                        float max_value, int zero_center, float* out, void* ws, cudaStream_t st);

@@ -286,3 +286,49 @@ int launch_subset_fill(const rsc_csr& X, const uint8_t* keep_rows, int32_t* out_
 }
 
 }  // namespace rsc
+
+// ------------------------------------------------------------------ NEXT-4 (part): HVG by cutoffs
+// mask_j = min_mean < m_j < max_mean and min_disp < z_j < max_disp (strict; NaN fails), the
+// selected genes listed in ascending order (one CTA: chunks of 1024 genes, ballot + running base)
+namespace rsc {
+
+__global__ void __launch_bounds__(1024)
+hvg_cutoffs_kernel(int32_t G, const double* __restrict__ mean_t, const double* __restrict__ disp_norm,
+                   double min_mean, double max_mean, double min_disp, double max_disp,
+                   uint8_t* __restrict__ out_mask, int32_t* __restrict__ out_idx, int32_t* __restrict__ out_count) {
+  __shared__ int wsum[32];
+  __shared__ int s_base;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) s_base = 0;
+  __syncthreads();
+  for (int c0 = 0; c0 < G; c0 += 1024) {
+    const int g = c0 + tid;
+    bool k = false;
+    if (g < G) {
+      const double m = mean_t[g], z = disp_norm[g];
+      k = m > min_mean && m < max_mean && z > min_disp && z < max_disp;
+      out_mask[g] = k ? 1 : 0;
+    }
+    const unsigned bal = __ballot_sync(0xffffffffu, k);
+    if (lane == 0) wsum[warp] = __popc(bal);
+    __syncthreads();
+    int off = s_base;
+    for (int w = 0; w < warp; ++w) off += wsum[w];
+    if (k && out_idx != nullptr) out_idx[off + __popc(bal & ((1u << lane) - 1u))] = g;
+    __syncthreads();
+    if (tid == 0) { int t = s_base; for (int w = 0; w < 32; ++w) t += wsum[w]; s_base = t; }
+    __syncthreads();
+  }
+  if (tid == 0) *out_count = s_base;
+}
+
+int launch_hvg_cutoffs(int32_t G, const double* mean_t, const double* disp_norm, double min_mean,
+                       double max_mean, double min_disp, double max_disp, uint8_t* out_mask,
+                       int32_t* out_idx, int32_t* out_count, cudaStream_t st) {
+  hvg_cutoffs_kernel<<<1, 1024, 0, st>>>(G, mean_t, disp_norm, min_mean, max_mean, min_disp, max_disp,
+                                         out_mask, out_idx, out_count);
+  RSC_LAUNCH_CHECK("hvg_cutoffs_kernel");
+  return RSC_OK;
+}
+
+}  // namespace rsc

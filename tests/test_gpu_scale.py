@@ -69,3 +69,23 @@ def test_chain_filter_hvg_subset_scale():
     yy = U.np_(y).astype(np.float64)[:, live]
     unclipped = np.abs(yy).max(axis=0) < 10.0                      # columns the clip did not touch
     np.testing.assert_allclose(yy[:, unclipped].mean(axis=0), 0, atol=1e-4)
+
+
+@pytest.mark.parametrize("G,seed", [(1, 0), (50, 1), (4099, 2), (36000, 3)])
+def test_hvg_cutoffs(G, seed):
+    """NEXT-4 (part): threshold-based selection on the device == the oracle's, bit-exact."""
+    from paper_2603_02402_b200 import binding as B
+    rng = np.random.default_rng(seed)
+    mean = np.exp(rng.normal(-3, 2, G)); var = mean * np.exp(rng.normal(0.2, 0.6, G))
+    mean[rng.random(G) < 0.1] = 0.0
+    h = B.rsc_hvg_select(torch.as_tensor(mean).cuda(), torch.as_tensor(var).cuda(), max(1, G // 10), 20, 1)
+    m, z = U.np_(h["mean_t"]), U.np_(h["disp_norm"])
+    for win in ((0.0125, 3.0, 0.5, np.inf), (-np.inf, np.inf, -np.inf, np.inf), (0.05, 0.05, 0.0, 1.0),
+                (0.0, 10.0, -0.25, 2.0)):
+        o = O.hvg_cutoffs(m, z, *win)
+        g = B.rsc_hvg_cutoffs(h["mean_t"], h["disp_norm"], *win)
+        torch.cuda.synchronize()
+        c = int(U.np_(g["count"])[0])
+        assert c == o["count"]
+        U.assert_int_equal(g["mask"], o["mask"], f"cutoff mask {win}")
+        assert np.array_equal(U.np_(g["indices"])[:c], o["indices"])
