@@ -63,8 +63,9 @@ typedef struct {
  * RSC_SPLIT_WIDTH) blocks; the table holds, for every row, K + 1 uint32 values
  *     splits[row * (K + 1) + k] = #{stored entries of the row with column < k * RSC_SPLIT_WIDTH}
  * (so splits[row][0] = 0 and splits[row][K] = the row length).  It is only meaningful for
- * rows with ascending column indices (RSC_CSR_SORTED).  rsc_qc_metrics can emit it for free
- * while it streams the matrix; rsc_row_splits computes it on its own (binary searches). */
+ * rows with ascending column indices (RSC_CSR_SORTED).  rsc_qc_metrics can emit it while it
+ * streams the matrix (binary searches in the row it has just read; rsc_qc_metrics_splits emits
+ * only chosen entries, which is cheaper); rsc_row_splits computes it on its own. */
 #define RSC_SPLIT_SHIFT 10
 #define RSC_SPLIT_WIDTH (1 << RSC_SPLIT_SHIFT)
 /* number of uint32 elements of the table */
