@@ -15,21 +15,30 @@
 //   * Segments are walked in 16-byte aligned quads: one 128-bit load per array and one
 //     128-bit store per lane; only the first / last quad of a segment can be partial and
 //     takes scalar accesses.
-//   * Accumulators: EXACT integer sums.  Only 32-bit integer shared atomics are native on
+//   * Accumulators: integer sums.  Only 32-bit integer shared atomics are native on
 //     sm_100 (ATOMS.ADD; 64-bit and floating-point ones are CAS loops), so a value v is
-//     first scaled by a power of two 2^k chosen (on the device, from the largest cell
-//     total) such that a = v * 2^k is an exact integer for every v >= 2^(23-k) -- the
-//     float32 significand has 24 bits -- and then
+//     first scaled by a power of two 2^k (chosen on the device) such that a = v * 2^k is an
+//     exact integer for every v >= 2^(23-k) -- the float32 significand has 24 bits.
+//     LINEAR-scale set (x', a 2^14-fold value range): 5 words per gene,
 //         S1 += a      as a 64-bit  integer in two   u32 words (w0, w1)
 //         S2 += a * a  as a 96-bit  integer in three u32 words (s0, s1, s2)
 //     where a word's carry-out (seen in the value the atomic returns) is added to the next
-//     word.  For 2^23 <= a < 2^32 (the usual case: a 512-fold range of v) the upper words
-//     only receive carries: ~3.1 atomics per entry and set.  a >= 2^32 takes the same path
-//     with 64-bit a (a < 2^42 by construction); v below the window (or negative / NaN) goes
-//     to the global double sums directly.  Integer adds commute, so the sums are exact and
-//     independent of the order of the adds; a flush (every <= 4092 rows, so no word can
-//     overflow) adds every word to its own 64-bit global counter, converted to double once at
-//     the end (fused_finish_kernel): bit-reproducible moments.
+//     word with a predicated increment: 2^23 <= a < 2^32 takes ~3.1 atomics per entry,
+//     2^32 <= a < 2^42 the same path with a two-word a.
+//     LOG-scale set (x'' = log1p(x') lies in [log1p(s / T_max), log1p(s)], a few binades):
+//     3 words per gene and NO branches -- window 2^23 <= a < 2^29 (64-fold),
+//         w0 += a                                  (returning atomic -> carry c1)
+//         s0 += low word of b,  b = (a*a + 2^13) >> 14   (returning atomic -> carry c0)
+//         W  += high word of b + c0 + (c1 << 23)   (one non-returning atomic)
+//     W packs the upper part of S2 (bits 0..22) and the carry count of S1 (bits 23..30);
+//     with at most 2040 rows between two flushes neither field can overflow.  S1 is exact;
+//     S2 is the sum of a*a rounded to a multiple of 2^14, i.e. to <= 2^-33 of the SMALLEST
+//     possible a*a (1.2e-10; 7e-12 for a typical x'' of 1..2) -- far inside the 1e-9 bar --
+//     and still an integer sum.  12 B / gene: 30 k genes need 2 groups, 18 k genes one.
+//     Values outside a set's window (or negative / NaN) go to the global double sums directly.
+//     Integer adds commute, so the on-chip sums do not depend on the order of the adds; a
+//     flush adds every word to its own 64-bit global counter, converted to double once at the
+//     end (fused_finish_kernel): bit-reproducible moments.
 //   * RSC_MOMENTS_FP64_ACC selects plain double accumulators (CAS atomics) instead: any
 //     value range, slower (fused_stream_fp64_kernel).
 #include <math.h>
@@ -49,7 +58,12 @@ constexpr int kFuThreads = RSC_FU_THREADS;
 #endif
 constexpr int kFuRowsPerGrab = RSC_FU_RG;
 constexpr int kMaxGroups = 64;
-constexpr int kSetWords = 5;               // u32 words per gene and moment set (w0 w1 s0 s1 s2)
+constexpr int kSetWords = 5;               // u32 words per gene of the linear-scale set (w0 w1 s0 s1 s2)
+constexpr int kLogWords = 3;               // u32 words per gene of the log-scale set (w0 s0 W)
+constexpr int kLogShift = 14;              // log-scale set: S2 accumulates (a * a + 2^13) >> 14
+constexpr int kLogBinades = 6;             // log-scale set: 2^23 <= a < 2^29
+constexpr int kLogCarryBit = 23;           // W = upper S2 word (bits 0..22) | carries of w0 (bits 23..30)
+constexpr int kLogRowBudget = 2040;        // rows between flushes: 2040 * 2^12 < 2^23, 2040 * 2^29 / 2^32 = 255
 constexpr double kRowCost = 200.0;         // per-row-segment overhead, in entries (plan kernel)
 constexpr int kMaxRangeBits = 19;          // 2^k * v_max <= 2^(23 + 19) = 2^42
 
@@ -188,7 +202,19 @@ fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid, f
     if (!(smin > 0.0) || !isfinite(smin)) smin = 1.0;
     if (smin > ts) smin = ts;
     plan->sc_lin = make_scale(smin, ts);
-    plan->sc_log = make_scale(log1p(smin), log1p(ts) * 1.000001);
+    {
+      // log-scale set: kLogBinades binades below the top 2^E > log1p(target_sum), the largest
+      // x'' non-negative data can produce
+      int E;
+      frexp(log1p(ts) * 1.000001, &E);
+      const int k = 23 - (E - kLogBinades);
+      MomentScale s;
+      s.mult = (float)ldexp(1.0, k);
+      s.pad = 0.0f;
+      s.inv1 = ldexp(1.0, -k);
+      s.inv2 = ldexp(1.0, kLogShift - 2 * k);
+      plan->sc_log = s;
+    }
   }
 }
 
@@ -277,6 +303,49 @@ __device__ __forceinline__ void acc_quad(uint32_t base, const uint32_t (&so)[4],
   for (int k = 0; k < 4; ++k) reds_inc_if(sa[k] + 16, carry_of(o[k], q1[k]) != 0u);
 }
 
+// ---- log-scale set: three words (w0 | s0 | W), branch-free
+// 2^23 <= t < 2^29
+__device__ __forceinline__ bool in_window_log(float t) {
+  return (__float_as_uint(t) - 0x4B000000u) < (uint32_t)kLogBinades * 0x00800000u;
+}
+// W increment: upper word of b + carry-out of (o0 + b0) + (carry-out of (o + a) << kLogCarryBit)
+__device__ __forceinline__ uint32_t log_top_word(uint32_t b1, uint32_t o0, uint32_t b0, uint32_t o, uint32_t a) {
+  return add_carry_of(b1, o0, b0) + (carry_of(o, a) << kLogCarryBit);
+}
+__device__ __forceinline__ void acc3_word(uint32_t sa, uint32_t a) {
+  unsigned long long q;
+  asm("mad.wide.u32 %0, %1, %1, %2;" : "=l"(q) : "r"(a), "l"(1ull << (kLogShift - 1)));
+  const uint32_t b0 = (uint32_t)(q >> kLogShift), b1 = (uint32_t)(q >> (32 + kLogShift));
+  const uint32_t o = atoms_add(sa, a);
+  const uint32_t o0 = atoms_add(sa + 4, b0);
+  reds_add(sa + 8, log_top_word(b1, o0, b0, o, a));
+}
+// the 4 entries of a quad, staged so that the returning atomics are in flight together; an
+// entry with a = 0 (masked) adds 0 to every word
+__device__ __forceinline__ void acc3_quad(uint32_t base, const uint32_t (&so)[4], const uint32_t (&a)[4]) {
+  uint32_t sa[4], o[4], o0[4], b0[4], b1[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { sa[k] = base + so[k]; o[k] = atoms_add(sa[k], a[k]); }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    unsigned long long q;
+    asm("mad.wide.u32 %0, %1, %1, %2;" : "=l"(q) : "r"(a[k]), "l"(1ull << (kLogShift - 1)));
+    b0[k] = (uint32_t)(q >> kLogShift); b1[k] = (uint32_t)(q >> (32 + kLogShift));
+    o0[k] = atoms_add(sa[k] + 4, b0[k]);
+  }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) reds_add(sa[k] + 8, log_top_word(b1[k], o0[k], b0[k], o[k], a[k]));
+}
+// log-scale value outside the fast path's reach
+__device__ __noinline__ void acc3_slow(uint32_t sa, float v, float mult, double* S1g, double* S2g) {
+  if (v == 0.0f) return;
+  const float t = v * mult;
+  if (in_window_log(t)) { acc3_word(sa, __float2uint_rz(t)); return; }
+  const double d = (double)v;                                      // outside the window, negative, NaN
+  atomicAdd(S1g, d);
+  atomicAdd(S2g, d * d);
+}
+
 // 2^23 <= t < 2^42: an exact integer of at most two words
 __device__ __forceinline__ bool in_window_wide(float t) {
   return (__float_as_uint(t) - 0x4B000000u) < 0x09800000u;       // 2^42 = 0x54800000
@@ -352,8 +421,8 @@ __device__ __noinline__ float entry_any(const AccCtx& c, int j, float x, float s
   const float xn = __fmul_rn(x, scale);
   const float xl = log1p_f32(xn);
   const uint32_t slot = min((uint32_t)(j - c.g0), c.last_slot);       // stays inside the table
-  if (LOG) acc_slow(c.sb_log + slot * (kSetWords * 4u), xl, c.mult_log, c.S1log + c.g0 + slot,
-                    c.S2log + c.g0 + slot);
+  if (LOG) acc3_slow(c.sb_log + slot * (kLogWords * 4u), xl, c.mult_log, c.S1log + c.g0 + slot,
+                     c.S2log + c.g0 + slot);
   if (LIN) acc_slow(c.sb_lin + slot * (kSetWords * 4u), xn, c.mult_lin, c.S1lin + c.g0 + slot,
                     c.S2lin + c.g0 + slot);
   return xl;
@@ -369,29 +438,35 @@ __device__ __noinline__ float4 quad_rare(const AccCtx& c, int4 jv, float4 xv, fl
   const float x[4] = {xv.x, xv.y, xv.z, xv.w};
   float xn[4], xl[4], tl[4], tn[4];
   bool ok = true;
-  uint32_t so[4];
+  uint32_t slot[4];
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
     const bool valid = (valid_mask >> k) & 1u;
     xn[k] = __fmul_rn(x[k], scale);
     xl[k] = log1p_ge_quarter(xn[k]);
     ok = ok && (xn[k] >= 0.25f || !valid);
-    if (LOG) { tl[k] = xl[k] * c.mult_log; ok = ok && (in_window_wide(tl[k]) || !valid); }
+    if (LOG) { tl[k] = xl[k] * c.mult_log; ok = ok && (in_window_log(tl[k]) || !valid); }
     if (LIN) { tn[k] = xn[k] * c.mult_lin; ok = ok && (in_window_wide(tn[k]) || !valid); }
-    const uint32_t slot = valid ? min((uint32_t)(j[k] - c.g0), c.last_slot) : spare_slot;
-    so[k] = slot * (kSetWords * 4u);
+    slot[k] = valid ? min((uint32_t)(j[k] - c.g0), c.last_slot) : spare_slot;
   }
-  if (ok) {
+  if (ok) {                     // only the linear-scale values need two words
     if (LOG) {
-      unsigned long long al[4];
+      uint32_t so[4], al[4];
 #pragma unroll
-      for (int k = 0; k < 4; ++k) al[k] = ((valid_mask >> k) & 1u) ? __float2ull_rz(tl[k]) : 0ull;
-      acc_quad_wide(c.sb_log, so, al);
+      for (int k = 0; k < 4; ++k) {
+        so[k] = slot[k] * (kLogWords * 4u);
+        al[k] = ((valid_mask >> k) & 1u) ? __float2uint_rz(tl[k]) : 0u;
+      }
+      acc3_quad(c.sb_log, so, al);
     }
     if (LIN) {
+      uint32_t so[4];
       unsigned long long an[4];
 #pragma unroll
-      for (int k = 0; k < 4; ++k) an[k] = ((valid_mask >> k) & 1u) ? __float2ull_rz(tn[k]) : 0ull;
+      for (int k = 0; k < 4; ++k) {
+        so[k] = slot[k] * (kSetWords * 4u);
+        an[k] = ((valid_mask >> k) & 1u) ? __float2ull_rz(tn[k]) : 0ull;
+      }
       acc_quad_wide(c.sb_lin, so, an);
     }
   } else {
@@ -426,19 +501,22 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
   const int ng_genes = min(a.n_cols, f1 << RSC_SPLIT_SHIFT) - g0;
   unsigned long long* counter = &a.plan->row_counter[grp];
 
-  // set s of slot g lives at fsm[(s * Gt + g) * 5 .. + 5): a stride of 5 words is odd, so the
-  // slots of a warp spread over all 32 banks
+  // log-scale set: slot g at fsm[g * 3 .. + 3); linear-scale set behind it: slot g at
+  // [Gt * 3 (if both) + g * 5 .. + 5).  Odd strides, so the slots of a warp spread over all 32
+  // banks.  The spare slot Gt of a set (masked entries add 0 there) is the first slot of
+  // whatever follows; the table ends with kSetWords spare words.
   AccCtx cx;
   {
     uint32_t sb = (uint32_t)__cvta_generic_to_shared(fsm);
     asm volatile("mov.u32 %0, %0;" : "+r"(sb));           // keep it in a register (no recomputation)
     cx.sb_log = sb;
-    cx.sb_lin = sb + (LOG ? (uint32_t)Gt * (kSetWords * 4u) : 0u);
+    cx.sb_lin = sb + (LOG ? (uint32_t)Gt * (kLogWords * 4u) : 0u);
   }
   cx.mult_log = mult_log; cx.mult_lin = mult_lin; cx.g0 = g0; cx.last_slot = (uint32_t)(Gt - 1);
   cx.S1log = a.S1log; cx.S2log = a.S2log; cx.S1lin = a.S1lin; cx.S2lin = a.S2lin;
   const uint32_t sb_log = cx.sb_log, sb_lin = cx.sb_lin, last_slot = cx.last_slot;
-  for (int i = tid; i < kSets * kSetWords * Gt + kSetWords; i += kFuThreads) fsm[i] = 0u;
+  constexpr int kWordsPerGene = (LOG ? kLogWords : 0) + (LIN ? kSetWords : 0);
+  for (int i = tid; i < kWordsPerGene * Gt + kSetWords; i += kFuThreads) fsm[i] = 0u;
 
   auto grab_issue = [&]() -> long long {                  // lane 0 only holds the result
     long long r = -1;
@@ -467,20 +545,21 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
       xn[k] = __fmul_rn(x[k], scale);
       xl[k] = log1p_ge_quarter(xn[k]);
       bool okk = xn[k] >= 0.25f;
-      if (LOG) { tl[k] = xl[k] * mult_log; okk = okk && in_window(tl[k]); }
+      if (LOG) { tl[k] = xl[k] * mult_log; okk = okk && in_window_log(tl[k]); }
       if (LIN) { tn[k] = xn[k] * mult_lin; okk = okk && in_window(tn[k]); }
       ok = ok && (okk || !valid[k]);
     }
     if (ok) {
-      uint32_t so[4], al[4], an[4];
+      uint32_t so[4], so3[4], al[4], an[4];
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         const uint32_t slot = valid[k] ? min((uint32_t)(j[k] - g0), last_slot) : (uint32_t)Gt;
-        so[k] = slot * (kSetWords * 4u);
+        if (LIN) so[k] = slot * (kSetWords * 4u);
+        if (LOG) so3[k] = slot * (kLogWords * 4u);
         if (LOG) al[k] = valid[k] ? __float2uint_rz(tl[k]) : 0u;
         if (LIN) an[k] = valid[k] ? __float2uint_rz(tn[k]) : 0u;
       }
-      if (LOG) acc_quad(sb_log, so, al);
+      if (LOG) acc3_quad(sb_log, so3, al);
       if (LIN) acc_quad(sb_lin, so, an);
     } else {
       const uint32_t vm = (valid[0] ? 1u : 0u) | (valid[1] ? 2u : 0u) | (valid[2] ? 4u : 0u) |
@@ -621,21 +700,31 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
       rnext = __shfl_sync(0xffffffffu, pending, 0);
     }
     done = __syncthreads_or(saw_end);
-    // flush this CTA's accumulators into the global integer totals and clear them
+    // flush this CTA's accumulators into the global integer totals and clear them: every
+    // 32-bit word is added to its own 64-bit counter (no carries between counters, so plain
+    // fire-and-forget atomics; a counter overflows only after 2^32 flushes): independent of
+    // the CTA order and of the grid
     for (int s = tid; s < ng_genes; s += kFuThreads) {
       const int g = g0 + s;
-#pragma unroll
-      for (int set = 0; set < kSets; ++set) {
-        const bool is_log = LOG && set == 0;
-        uint32_t* w = fsm + ((size_t)set * Gt + s) * kSetWords;
+      const size_t G64 = (size_t)a.n_cols;
+      if (LOG) {
+        uint32_t* w = fsm + (size_t)s * kLogWords;
+        const uint32_t w0 = w[0], s0 = w[1], W = w[2];
+        if (w0 | s0 | W) {
+          unsigned long long* acc = a.acc_log + g;
+          // S1 words: w0 and its carry count; S2 words: s0 and the upper field of W
+          atomicAdd(acc, ((unsigned long long)(W >> kLogCarryBit) << 32) | w0);
+          if (s0) atomicAdd(acc + 2 * G64, (unsigned long long)s0);
+          if (W & ((1u << kLogCarryBit) - 1u))
+            atomicAdd(acc + 3 * G64, (unsigned long long)(W & ((1u << kLogCarryBit) - 1u)));
+          w[0] = 0u; w[1] = 0u; w[2] = 0u;
+        }
+      }
+      if (LIN) {
+        uint32_t* w = fsm + (LOG ? (size_t)Gt * kLogWords : 0) + (size_t)s * kSetWords;
         const uint32_t w0 = w[0], w1 = w[1], s0 = w[2], s1 = w[3], s2 = w[4];
         if (w0 | w1 | s0 | s1 | s2) {
-          // integer totals in global memory: every 32-bit word of the CTA's sums is added to
-          // its own 64-bit counter (no carries between counters, so plain fire-and-forget
-          // atomics; a counter overflows only after 2^32 flushes): exact, and independent of
-          // the CTA order and of the grid
-          unsigned long long* acc = (is_log ? a.acc_log : a.acc_lin) + g;
-          const size_t G64 = (size_t)a.n_cols;
+          unsigned long long* acc = a.acc_lin + g;
           if (w0) atomicAdd(acc, (unsigned long long)w0);
           if (w1) atomicAdd(acc + G64, (unsigned long long)w1);
           if (s0) atomicAdd(acc + 2 * G64, (unsigned long long)s0);
@@ -752,7 +841,8 @@ static int fused_grid() { return g_opt.grid_ctas > 0 ? g_opt.grid_ctas : sm_coun
 // bytes of shared-memory accumulators per gene
 static int bytes_per_gene(int which) {
   const int sets = ((which & RSC_MOMENTS_LOG) ? 1 : 0) + ((which & RSC_MOMENTS_LIN) ? 1 : 0);
-  return sets * ((which & RSC_MOMENTS_FP64_ACC) ? 16 : kSetWords * 4);
+  if (which & RSC_MOMENTS_FP64_ACC) return sets * 16;
+  return ((which & RSC_MOMENTS_LOG) ? kLogWords * 4 : 0) + ((which & RSC_MOMENTS_LIN) ? kSetWords * 4 : 0);
 }
 
 // column blocks per group: as many as fit, then evened out over the groups
@@ -844,6 +934,8 @@ int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i
     a.indptr = X.indptr; a.indices = X.indices; a.data = X.data; a.cell_total = cell_total_i64;
     a.splits = row_splits; a.target_sum = target_sum;
     a.row_budget = (uint32_t)g_opt.fused_row_budget;
+    if ((which & RSC_MOMENTS_LOG) && !(which & RSC_MOMENTS_FP64_ACC) && a.row_budget > (uint32_t)kLogRowBudget)
+      a.row_budget = (uint32_t)kLogRowBudget;                    // the packed word W of the log-scale set
     a.S1log = S1log; a.S2log = S2log; a.S1lin = S1lin; a.S2lin = S2lin; a.plan = plan;
     const bool int_acc = !(which & RSC_MOMENTS_FP64_ACC);
     a.acc_log = reinterpret_cast<unsigned long long*>(accb);
