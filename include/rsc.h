@@ -79,9 +79,12 @@ const char* rsc_version(void);
  * counter; memsets / memcpys are not counted).  Used by bench.py to report gpu_launches. */
 uint64_t rsc_kernel_launch_count(void);
 /* Process-wide tuning / testing knobs (not needed in normal use; defaults in brackets):
- *   "fused_row_budget" [4000]  rows a CTA of the fused pass takes between two flushes of its
- *                              integer accumulators (1..4092; 4096 rows cannot overflow)
- *   "qc_row_budget"    [2043]  the same for the QC pass's 11-bit count fields (1..2043)
+ *   "fused_row_budget" [512]   rows a CTA of the fused pass takes between two checks of its
+ *                              integer accumulator tables (1..512, rounded down to a power of
+ *                              two); a check moves the genes whose words are half full to the
+ *                              global totals
+ *   "flush_all"        [0]     1 = every check moves EVERY gene (testing the exchange path)
+ *   "qc_row_budget"    [512]   the same for the QC pass's packed count | total words (1..512)
  *   "grid_ctas"        [0]     CTAs of the streaming kernels, 0 = one per SM
  *   "force_generic"    [0]     1 = always take the generic L2-atomic kernels
  * Returns RSC_ERR_INVALID_ARG for an unknown key or a value out of range. */

@@ -96,10 +96,12 @@ uint64_t rsc_kernel_launch_count(void) { return g_launch_count; }
 int rsc_set_option(const char* key, long long value) {
   RSC_CHECK_ARG(key != nullptr, "rsc_set_option: key is NULL");
   if (!strcmp(key, "fused_row_budget")) {
-    RSC_CHECK_ARG(value >= 1 && value <= 4092, "rsc_set_option: fused_row_budget must be in [1, 4092]");
+    RSC_CHECK_ARG(value >= 1 && value <= 512, "rsc_set_option: fused_row_budget must be in [1, 512]");
     g_opt.fused_row_budget = (int)value;
+  } else if (!strcmp(key, "flush_all")) {
+    g_opt.flush_all = value != 0;
   } else if (!strcmp(key, "qc_row_budget")) {
-    RSC_CHECK_ARG(value >= 1 && value <= 2043, "rsc_set_option: qc_row_budget must be in [1, 2043]");
+    RSC_CHECK_ARG(value >= 1 && value <= 512, "rsc_set_option: qc_row_budget must be in [1, 512]");
     g_opt.qc_row_budget = (int)value;
   } else if (!strcmp(key, "grid_ctas")) {
     RSC_CHECK_ARG(value >= 0 && value <= 65535, "rsc_set_option: grid_ctas must be in [0, 65535]");

@@ -39,8 +39,9 @@ void set_error(const char* fmt, ...);
 
 // run-time tunables (rsc_set_option): defaults are the shipped configuration
 struct Options {
-  int fused_row_budget = 4000;    // rows a fused-pass CTA takes between flushes (<= 4092)
-  int qc_row_budget = 2043;       // rows a QC CTA takes between flushes (<= 2047 - 4)
+  int fused_row_budget = 512;     // rows a fused-pass CTA takes between two checks of its tables (<= 512)
+  int flush_all = 0;              // 1: every check moves every gene to the global totals (testing)
+  int qc_row_budget = 512;        // rows a QC CTA takes between two checks of its table (<= 512)
   int grid_ctas = 0;              // CTAs of the streaming kernels; 0 = one per SM
   int force_generic = 0;          // 1: always use the generic L2-atomic kernels
 };

@@ -54,16 +54,21 @@ namespace rsc {
 #endif
 constexpr int kFuThreads = RSC_FU_THREADS;
 #ifndef RSC_FU_RG
-#define RSC_FU_RG 4
+#define RSC_FU_RG 2
 #endif
 constexpr int kFuRowsPerGrab = RSC_FU_RG;
+constexpr long long kCheckBit = 1LL << 62;  // set in a grab's result: this grab crossed a check point
 constexpr int kMaxGroups = 64;
+// rows a CTA can add between two checks of a gene: the check interval (<= 512) + the grabs its
+// warps hold (current, next, pending) must stay below 1020 (see check_tables)
+static_assert(512 + 3 * (kFuThreads / 32) * kFuRowsPerGrab + 64 <= 1020, "fused pass: too many rows in flight for the lazy flush");
 constexpr int kSetWords = 5;               // u32 words per gene of the linear-scale set (w0 w1 s0 s1 s2)
 constexpr int kLogWords = 3;               // u32 words per gene of the log-scale set (w0 s0 W)
 constexpr int kLogShift = 14;              // log-scale set: S2 accumulates (a * a + 2^13) >> 14
 constexpr int kLogBinades = 6;             // log-scale set: 2^23 <= a < 2^29
 constexpr int kLogCarryBit = 23;           // W = upper S2 word (bits 0..22) | carries of w0 (bits 23..30)
-constexpr int kLogRowBudget = 2040;        // rows between flushes: 2040 * 2^12 < 2^23, 2040 * 2^29 / 2^32 = 255
+// a gene is moved out when a field of W is half full and checked at least every 1020 rows:
+// 1020 * 2^12 < 2^22 (upper S2 word), 1020 * 2^29 / 2^32 + 1 <= 128 (carries of w0)
 constexpr double kRowCost = 200.0;         // per-row-segment overhead, in entries (plan kernel)
 constexpr int kMaxRangeBits = 19;          // 2^k * v_max <= 2^(23 + 19) = 2^42
 
@@ -96,7 +101,9 @@ struct FusedArgs {
   const int64_t* cell_total;
   const uint32_t* splits;
   float target_sum;
-  uint32_t row_budget;       // a CTA stops grabbing rows once it has taken this many (then flushes)
+  uint32_t row_budget;       // fp64 kernel: a CTA stops grabbing rows once it has taken this many (then flushes)
+  uint32_t check_shift;      // integer kernels: a warp checks the CTA's tables every 2^check_shift rows
+  uint32_t flush_all;        // 1: a check moves every gene to the global totals (testing)
   double* S1log; double* S2log; double* S1lin; double* S2lin;
   unsigned long long* acc_log;   // [5][n_cols] global totals of the words w0 w1 s0 s1 s2
   unsigned long long* acc_lin;
@@ -205,9 +212,12 @@ fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid, f
     {
       // log-scale set: kLogBinades binades below the top 2^E > log1p(target_sum), the largest
       // x'' non-negative data can produce
+      // (and never below 2^-2: log1p_ge_quarter of an x' < 0.25 is < 0.2232, so such a value
+      // fails the window test by itself and the log-only kernel needs no separate x' test)
       int E;
       frexp(log1p(ts) * 1.000001, &E);
-      const int k = 23 - (E - kLogBinades);
+      const int L = max(E - kLogBinades, -2);
+      const int k = 23 - L;
       MomentScale s;
       s.mult = (float)ldexp(1.0, k);
       s.pad = 0.0f;
@@ -518,13 +528,67 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
   constexpr int kWordsPerGene = (LOG ? kLogWords : 0) + (LIN ? kSetWords : 0);
   for (int i = tid; i < kWordsPerGene * Gt + kSetWords; i += kFuThreads) fsm[i] = 0u;
 
-  auto grab_issue = [&]() -> long long {                  // lane 0 only holds the result
-    long long r = -1;
+  // Row grabs (lane 0 only holds the result).  s_rows counts the rows this CTA has taken; the
+  // warp whose grab crosses a multiple of 2^check_shift checks the tables (bit 62 of the result).
+  auto grab_issue = [&]() -> long long {
+    long long r = 0;
     if (lane == 0) {
       const unsigned c = atomicAdd(&s_rows, (unsigned)kFuRowsPerGrab);
-      if (c < a.row_budget) r = (long long)atomicAdd(counter, (unsigned long long)kFuRowsPerGrab);
+      r = (long long)atomicAdd(counter, (unsigned long long)kFuRowsPerGrab);
+      if (((c ^ (c + (unsigned)kFuRowsPerGrab)) >> a.check_shift) != 0u) r |= kCheckBit;
     }
     return r;
+  };
+  // A gene's words leave the CTA as 64-bit adds to the global integer totals: every 32-bit
+  // word goes to its own counter (no carries between counters, so plain fire-and-forget
+  // atomics; a counter overflows only after 2^32 flushes) -- independent of the CTA order and
+  // of the grid.
+  auto to_global_log = [&](int g, uint32_t w0, uint32_t s0, uint32_t W) {
+    unsigned long long* acc = a.acc_log + g;
+    const size_t G64 = (size_t)a.n_cols;
+    const uint32_t hi = W & ((1u << kLogCarryBit) - 1u);
+    // S1: w0 and its carry count in one add; S2: s0 and the upper field of W
+    atomicAdd(acc, ((unsigned long long)(W >> kLogCarryBit) << 32) | w0);
+    if (s0) atomicAdd(acc + 2 * G64, (unsigned long long)s0);
+    if (hi) atomicAdd(acc + 3 * G64, (unsigned long long)hi);
+  };
+  auto to_global_lin = [&](int g, uint32_t w0, uint32_t w1, uint32_t s0, uint32_t s1, uint32_t s2) {
+    unsigned long long* acc = a.acc_lin + g;
+    const size_t G64 = (size_t)a.n_cols;
+    if (w0) atomicAdd(acc, (unsigned long long)w0);
+    if (w1) atomicAdd(acc + G64, (unsigned long long)w1);
+    if (s0) atomicAdd(acc + 2 * G64, (unsigned long long)s0);
+    if (s1) atomicAdd(acc + 3 * G64, (unsigned long long)s1);
+    if (s2) atomicAdd(acc + 4 * G64, (unsigned long long)s2);
+  };
+  // Table check by ONE warp while the others keep adding: a gene whose packed word W (log
+  // set) or top word (linear set) is at least half full is moved to the global totals, word
+  // by word with an atomic exchange.  Each word is an independent sum (a carry is computed by
+  // the adder from the value ITS atomic returned), so exchanging a word to 0 between two
+  // adds loses nothing.  Between two checks of a gene a CTA adds at most
+  // 2^check_shift + (rows in flight) < 1020 rows, i.e. less than half of any field.
+  auto check_tables = [&]() {
+    for (int s = lane; s < ng_genes; s += 32) {
+      if (LOG) {
+        uint32_t* w = fsm + (size_t)s * kLogWords;
+        const uint32_t W = *reinterpret_cast<volatile uint32_t*>(w + 2);
+        if (a.flush_all || (W & ((1u << kLogCarryBit) - 1u)) >= (1u << (kLogCarryBit - 1)) ||
+            (W >> kLogCarryBit) >= 128u) {
+          const uint32_t w0 = atomicExch(w, 0u), s0 = atomicExch(w + 1, 0u), Wx = atomicExch(w + 2, 0u);
+          if (w0 | s0 | Wx) to_global_log(g0 + s, w0, s0, Wx);
+        }
+      }
+      if (LIN) {
+        uint32_t* w = fsm + (LOG ? (size_t)Gt * kLogWords : 0) + (size_t)s * kSetWords;
+        const uint32_t w1 = *reinterpret_cast<volatile uint32_t*>(w + 1);
+        const uint32_t s2 = *reinterpret_cast<volatile uint32_t*>(w + 4);
+        if (a.flush_all || ((w1 | s2) >> 31) != 0u) {
+          const uint32_t x0 = atomicExch(w, 0u), x1 = atomicExch(w + 1, 0u), y0 = atomicExch(w + 2, 0u),
+                         y1 = atomicExch(w + 3, 0u), y2 = atomicExch(w + 4, 0u);
+          if (x0 | x1 | y0 | y1 | y2) to_global_lin(g0 + s, x0, x1, y0, y1, y2);
+        }
+      }
+    }
   };
 
   // One quad of 4 consecutive entries.  Straight-line code when every value is in the usual
@@ -544,7 +608,7 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
       valid[k] = !EDGE || (unsigned)(e0 + k) < (unsigned)len;
       xn[k] = __fmul_rn(x[k], scale);
       xl[k] = log1p_ge_quarter(xn[k]);
-      bool okk = xn[k] >= 0.25f;
+      bool okk = (LOG && !LIN) || xn[k] >= 0.25f;       // log only: implied by the window test
       if (LOG) { tl[k] = xl[k] * mult_log; okk = okk && in_window_log(tl[k]); }
       if (LIN) { tn[k] = xn[k] * mult_lin; okk = okk && in_window(tn[k]); }
       ok = ok && (okk || !valid[k]);
@@ -569,11 +633,9 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
     return make_float4(xl[0], xl[1], xl[2], xl[3]);
   };
 
-  int done;
-  do {
+  {
     if (tid == 0) s_rows = 0u;
     __syncthreads();
-    int saw_end = 0;
     // Grabs are pipelined two deep: while grab g is processed, the row range of grab g + 1 is
     // already known, its row metadata is loaded and its segments are prefetched into L2, and
     // the atomic for grab g + 2 is in flight -- no latency chain between grabs.
@@ -596,15 +658,14 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
         asm volatile("prefetch.global.L2 [%0];" ::"l"(a.data + p));
       }
     };
-    long long r0 = __shfl_sync(0xffffffffu, grab_issue(), 0);
+    long long r0 = __shfl_sync(0xffffffffu, grab_issue(), 0) & ~kCheckBit;
     int64_t mbeg = 0, mend = 0;
     float mscale = 1.0f;
-    if (r0 >= 0 && r0 < a.n_rows) load_meta(r0, mbeg, mend, mscale);
-    long long rnext = __shfl_sync(0xffffffffu, grab_issue(), 0);
-    while (r0 >= 0) {
-      if (r0 >= a.n_rows) { saw_end = 1; break; }
+    if (r0 < a.n_rows) load_meta(r0, mbeg, mend, mscale);
+    long long rnext = __shfl_sync(0xffffffffu, grab_issue(), 0) & ~kCheckBit;
+    while (r0 < a.n_rows) {
       const long long pending = grab_issue();             // grab g + 2; consumed after this grab
-      const bool next_ok = rnext >= 0 && rnext < a.n_rows;
+      const bool next_ok = rnext < a.n_rows;
       int64_t nbeg = 0, nend = 0;
       float nscale = 1.0f;
       if (next_ok) load_meta(rnext, nbeg, nend, nscale);
@@ -698,43 +759,21 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
       }
       r0 = rnext; mbeg = nbeg; mend = nend; mscale = nscale;
       rnext = __shfl_sync(0xffffffffu, pending, 0);
+      if (rnext & kCheckBit) { rnext &= ~kCheckBit; check_tables(); }
     }
-    done = __syncthreads_or(saw_end);
-    // flush this CTA's accumulators into the global integer totals and clear them: every
-    // 32-bit word is added to its own 64-bit counter (no carries between counters, so plain
-    // fire-and-forget atomics; a counter overflows only after 2^32 flushes): independent of
-    // the CTA order and of the grid
+    __syncthreads();
+    // the matrix is exhausted: everything left in the tables goes to the global totals
     for (int s = tid; s < ng_genes; s += kFuThreads) {
-      const int g = g0 + s;
-      const size_t G64 = (size_t)a.n_cols;
       if (LOG) {
-        uint32_t* w = fsm + (size_t)s * kLogWords;
-        const uint32_t w0 = w[0], s0 = w[1], W = w[2];
-        if (w0 | s0 | W) {
-          unsigned long long* acc = a.acc_log + g;
-          // S1 words: w0 and its carry count; S2 words: s0 and the upper field of W
-          atomicAdd(acc, ((unsigned long long)(W >> kLogCarryBit) << 32) | w0);
-          if (s0) atomicAdd(acc + 2 * G64, (unsigned long long)s0);
-          if (W & ((1u << kLogCarryBit) - 1u))
-            atomicAdd(acc + 3 * G64, (unsigned long long)(W & ((1u << kLogCarryBit) - 1u)));
-          w[0] = 0u; w[1] = 0u; w[2] = 0u;
-        }
+        const uint32_t* w = fsm + (size_t)s * kLogWords;
+        if (w[0] | w[1] | w[2]) to_global_log(g0 + s, w[0], w[1], w[2]);
       }
       if (LIN) {
-        uint32_t* w = fsm + (LOG ? (size_t)Gt * kLogWords : 0) + (size_t)s * kSetWords;
-        const uint32_t w0 = w[0], w1 = w[1], s0 = w[2], s1 = w[3], s2 = w[4];
-        if (w0 | w1 | s0 | s1 | s2) {
-          unsigned long long* acc = a.acc_lin + g;
-          if (w0) atomicAdd(acc, (unsigned long long)w0);
-          if (w1) atomicAdd(acc + G64, (unsigned long long)w1);
-          if (s0) atomicAdd(acc + 2 * G64, (unsigned long long)s0);
-          if (s1) atomicAdd(acc + 3 * G64, (unsigned long long)s1);
-          if (s2) atomicAdd(acc + 4 * G64, (unsigned long long)s2);
-          w[0] = 0u; w[1] = 0u; w[2] = 0u; w[3] = 0u; w[4] = 0u;
-        }
+        const uint32_t* w = fsm + (LOG ? (size_t)Gt * kLogWords : 0) + (size_t)s * kSetWords;
+        if (w[0] | w[1] | w[2] | w[3] | w[4]) to_global_lin(g0 + s, w[0], w[1], w[2], w[3], w[4]);
       }
     }
-  } while (!done);
+  }
 }
 
 // ------------------------------------------------------------------ double accumulators
@@ -933,9 +972,10 @@ int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i
     a.Gt = a.fine_per_group * RSC_SPLIT_WIDTH;
     a.indptr = X.indptr; a.indices = X.indices; a.data = X.data; a.cell_total = cell_total_i64;
     a.splits = row_splits; a.target_sum = target_sum;
-    a.row_budget = (uint32_t)g_opt.fused_row_budget;
-    if ((which & RSC_MOMENTS_LOG) && !(which & RSC_MOMENTS_FP64_ACC) && a.row_budget > (uint32_t)kLogRowBudget)
-      a.row_budget = (uint32_t)kLogRowBudget;                    // the packed word W of the log-scale set
+    a.row_budget = 4000u;
+    a.check_shift = 0u;                                         // largest power of two <= the option (<= 512)
+    while (a.check_shift < 9u && (2u << a.check_shift) <= (uint32_t)g_opt.fused_row_budget) ++a.check_shift;
+    a.flush_all = g_opt.flush_all ? 1u : 0u;
     a.S1log = S1log; a.S2log = S2log; a.S1lin = S1lin; a.S2lin = S2lin; a.plan = plan;
     const bool int_acc = !(which & RSC_MOMENTS_FP64_ACC);
     a.acc_log = reinterpret_cast<unsigned long long*>(accb);

@@ -9,8 +9,11 @@
 //         bits 20..30 n_cells_j of this flush period   (11 bits)
 //         bits 0..19  total_j of this flush period     (20 bits)
 //     Entries with a count > 511 (or negative / beyond the table) bypass the table and go to
-//     the global outputs directly.  A CTA flushes its table after at most 2047 rows
-//     (2047 * 511 < 2^20), so no field can overflow into its neighbour;
+//     the global outputs directly.  Every 512 rows of the CTA one warp checks the table and
+//     moves the genes whose count or total field is half full to the global outputs (one
+//     atomic AND per gene, while the other warps keep adding); fewer than 1020 rows are added
+//     between two checks of a gene (1020 * 511 < 2^19), so no field can overflow into its
+//     neighbour.  Whatever is left goes out once, at the end;
 //   * optionally the row split table consumed by the fused pass (fused.cu): for every row,
 //     the number of entries with column < k * RSC_SPLIT_WIDTH, found by comparing the column
 //     block of a lane's last entry with its neighbour's (rows must be sorted).
@@ -34,14 +37,15 @@ constexpr int kQcRowsPerGrab = RSC_QC_RG;
 #endif
 constexpr int kQcAhead = RSC_QC_AHEAD;                  // L2 look-ahead of a warp, in steps of 128 entries
 constexpr uint32_t kQcMaxFast = 511u;        // largest count that takes the shared-memory path
-constexpr int kQcMaxRowBudget = 2047 - kQcRowsPerGrab;   // rows per flush period incl. the last grab
+static_assert(512 + 3 * kQcWarps * kQcRowsPerGrab + 64 <= 1020, "QC pass: too many rows in flight for the lazy flush");
 
 struct QcArgs {
   int64_t n_rows;
   int64_t nnz;
   int32_t n_cols;
   int32_t n_fine;            // K = number of column blocks (split table has K + 1 entries per row)
-  uint32_t row_budget;       // a CTA stops grabbing rows once it has taken this many (then flushes)
+  uint32_t check_shift;      // a warp checks the CTA's table every 2^check_shift rows
+  uint32_t flush_all;        // 1: a check moves every gene to the global outputs (testing)
   const int64_t* indptr;
   const int32_t* indices;
   const float* data;
@@ -72,6 +76,25 @@ __device__ __forceinline__ uint32_t qc_atoms_add(uint32_t saddr, uint32_t v) {
   return old;
 }
 
+// count | total of one packed word -> the global outputs
+__device__ __forceinline__ void qc_word_to_global(int g, uint32_t w, int32_t* gene_n_cells,
+                                                  unsigned long long* gene_total) {
+  const uint32_t c = (w >> 20) & 0x7ffu, t = w & 0xfffffu;
+  if (c != 0u && gene_n_cells != nullptr) atomicAdd(&gene_n_cells[g], (int)c);
+  if (t != 0u && gene_total != nullptr) atomicAdd(&gene_total[g], (unsigned long long)t);
+}
+// Table check by one warp while the others keep adding: genes with a half-full field leave
+// the table (atomic AND: the flag bit stays, the old word is what goes out).  Out of line:
+// it runs once per 512 rows and must not cost the streaming loop registers.
+__device__ __noinline__ void qc_check_table(uint32_t* qsm, int G, int lane, uint32_t flush_all,
+                                            int32_t* gene_n_cells, unsigned long long* gene_total) {
+  for (int g = lane; g < G; g += 32) {
+    const uint32_t w = *reinterpret_cast<volatile uint32_t*>(qsm + g);
+    if (flush_all || (w & 0x40000000u) != 0u || (w & 0x80000u) != 0u)
+      qc_word_to_global(g, atomicAnd(qsm + g, 0x80000000u), gene_n_cells, gene_total);
+  }
+}
+
 template <bool SPLITS>
 __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a) {
   extern __shared__ __align__(16) uint32_t qsm[];      // [G] packed flag | count | total, + 1 spare
@@ -81,21 +104,26 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
   uint32_t sbase = (uint32_t)__cvta_generic_to_shared(qsm);
   asm volatile("mov.u32 %0, %0;" : "+r"(sbase));       // keep it in a register
   __shared__ unsigned s_rows;
+  __shared__ volatile unsigned s_chk;
 
   for (int g = tid; g <= G; g += kQcThreads)
     qsm[g] = (g < G && a.flags != nullptr && a.flags[g] != 0) ? 0x80000000u : 0u;
 
-  // -1: the CTA's row budget is used up (flush first); >= n_rows: the matrix is exhausted
-  // (only lane 0 holds the result; it is broadcast when needed)
+  // Row grabs: >= n_rows means the matrix is exhausted (only lane 0 holds the result; it is
+  // broadcast when needed).  s_rows counts the rows this CTA has taken; the warp whose grab
+  // crosses a multiple of 2^check_shift raises s_chk; the next warp to finish a grab takes it
+  // and checks the table.
   auto grab_issue = [&]() -> long long {
-    long long r = -1;
+    long long r = 0;
     if (lane == 0) {
       const unsigned c = atomicAdd(&s_rows, (unsigned)kQcRowsPerGrab);
-      if (c < a.row_budget)
-        r = (long long)atomicAdd(a.row_counter, (unsigned long long)kQcRowsPerGrab);
+      r = (long long)atomicAdd(a.row_counter, (unsigned long long)kQcRowsPerGrab);
+      if (((c ^ (c + (unsigned)kQcRowsPerGrab)) >> a.check_shift) != 0u) s_chk = 1u;
     }
     return r;
   };
+  auto to_global = [&](int g, uint32_t w) { qc_word_to_global(g, w, a.gene_n_cells, a.gene_total); };
+  auto check_table = [&]() { qc_check_table(qsm, G, lane, a.flush_all, a.gene_n_cells, a.gene_total); };
   auto load_ptrs = [&](long long r0) -> int64_t {       // lanes 0..RG: indptr[r0 + lane]
     int64_t p = 0;
     if (lane <= kQcRowsPerGrab && r0 + lane <= a.n_rows) p = a.indptr[r0 + lane];
@@ -169,21 +197,18 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
     }
   };
 
-  int done;
-  do {
-    if (tid == 0) s_rows = 0u;
+  {
+    if (tid == 0) { s_rows = 0u; s_chk = 0u; }
     __syncthreads();
-    int saw_end = 0;
     // Grabs are pipelined two deep (see fused.cu): row range of grab g + 1 known and its
     // indptr entries loaded while grab g is processed; every row is prefetched into L2 one
     // row ahead of its use.
     long long r0 = __shfl_sync(0xffffffffu, grab_issue(), 0);
-    int64_t mptr = (r0 >= 0 && r0 < a.n_rows) ? load_ptrs(r0) : 0;
+    int64_t mptr = r0 < a.n_rows ? load_ptrs(r0) : 0;
     long long rnext = __shfl_sync(0xffffffffu, grab_issue(), 0);
-    while (r0 >= 0) {
-      if (r0 >= a.n_rows) { saw_end = 1; break; }
+    while (r0 < a.n_rows) {
       const long long pending = grab_issue();
-      const bool next_ok = rnext >= 0 && rnext < a.n_rows;
+      const bool next_ok = rnext < a.n_rows;
       const int64_t nptr = next_ok ? load_ptrs(rnext) : 0;
       const int nr = (int)min((long long)kQcRowsPerGrab, a.n_rows - r0);
       const int64_t gend = __shfl_sync(0xffffffffu, mptr, nr);   // end of the grab's contiguous range
@@ -273,19 +298,16 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
       }
       r0 = rnext; mptr = nptr;
       rnext = __shfl_sync(0xffffffffu, pending, 0);
-    }
-    done = __syncthreads_or(saw_end);
-    // flush and clear the CTA's table (the flag bit stays)
-    for (int g = tid; g < G; g += kQcThreads) {
-      const uint32_t w = qsm[g];
-      const uint32_t c = (w >> 20) & 0x7ffu, t = w & 0xfffffu;
-      if (c | t) {
-        if (c != 0u && a.gene_n_cells != nullptr) atomicAdd(&a.gene_n_cells[g], (int)c);
-        if (t != 0u && a.gene_total != nullptr) atomicAdd(&a.gene_total[g], (unsigned long long)t);
-        qsm[g] = w & 0x80000000u;
+      if (s_chk != 0u) {
+        unsigned t = 0u;
+        if (lane == 0) t = atomicExch(const_cast<unsigned*>(&s_chk), 0u);
+        if (__shfl_sync(0xffffffffu, t, 0) != 0u) check_table();
       }
     }
-  } while (!done);
+    __syncthreads();
+    // the matrix is exhausted: what is left in the table goes to the global outputs
+    for (int g = tid; g < G; g += kQcThreads) to_global(g, qsm[g]);
+  }
 }
 
 // ------------------------------------------------------------------ standalone split table
@@ -378,7 +400,9 @@ int launch_qc(const rsc_csr& X, const uint8_t* gene_flags, int64_t* cell_total_i
                                   (int)kMaxDynSmem));
     attr_set = true;
   }
-  a.row_budget = (uint32_t)min(g_opt.qc_row_budget, kQcMaxRowBudget);
+  a.check_shift = 0u;                                           // largest power of two <= the option (<= 512)
+  while (a.check_shift < 9u && (2u << a.check_shift) <= (uint32_t)g_opt.qc_row_budget) ++a.check_shift;
+  a.flush_all = g_opt.flush_all ? 1u : 0u;
   int64_t blocks = (X.n_rows + kQcWarps * kQcRowsPerGrab - 1) / (kQcWarps * kQcRowsPerGrab);
   const int cap = g_opt.grid_ctas > 0 ? g_opt.grid_ctas : sm_count();
   if (blocks > cap) blocks = cap;

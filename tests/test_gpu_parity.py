@@ -304,11 +304,13 @@ def small_budgets():
     """Force many flushes of the CTA-private tables and a small grid (rsc_set_option)."""
     from paper_2603_02402_b200 import binding as B
     B.rsc_set_option("fused_row_budget", 8)
+    B.rsc_set_option("flush_all", 1)
     B.rsc_set_option("qc_row_budget", 8)
     B.rsc_set_option("grid_ctas", 9)
     yield
-    B.rsc_set_option("fused_row_budget", 4000)
-    B.rsc_set_option("qc_row_budget", 2043)
+    B.rsc_set_option("fused_row_budget", 512)
+    B.rsc_set_option("flush_all", 0)
+    B.rsc_set_option("qc_row_budget", 512)
     B.rsc_set_option("grid_ctas", 0)
 
 
