@@ -980,7 +980,9 @@ int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i
     const bool int_acc = !(which & RSC_MOMENTS_FP64_ACC);
     a.acc_log = reinterpret_cast<unsigned long long*>(accb);
     a.acc_lin = reinterpret_cast<unsigned long long*>(accb + asz);
-    {
+    if ((which & RSC_MOMENTS_LIN) && !(which & RSC_MOMENTS_FP64_ACC)) {
+      // the largest cell total places the linear-scale window (the log-scale one hangs from
+      // log1p(target_sum) and needs nothing from the data)
       int64_t blocks = (X.n_rows + 255) / 256;
       const int64_t cap = (int64_t)sm_count() * 4;
       if (blocks > cap) blocks = cap;
