@@ -70,6 +70,17 @@ int launch_qc_generic(const rsc_csr& X, const uint8_t* gene_flags, int64_t* cell
 }
 
 // ------------------------------------------------------------------ normalize_total
+// x' = x * scale_i in place: 4 B read + 4 B written per stored entry.  A warp per
+// row; the row is walked as 16-byte aligned float4's (scalar head / tail of at most 3
+// elements), four per lane in flight.  Without supplied totals the row is summed first (fp64;
+// the second sweep finds it in L1 / L2).
+__device__ __forceinline__ void row_vec_bounds(const float* rowp, int64_t len, int& head, int64_t& nvec) {
+  const uintptr_t a = reinterpret_cast<uintptr_t>(rowp);
+  const int64_t h = ((16 - (a & 15)) & 15) >> 2;
+  head = (int)(h < len ? h : len);
+  nvec = (len - head) >> 2;
+}
+
 __global__ void __launch_bounds__(256)
 normalize_kernel(int64_t n_rows, const int64_t* __restrict__ indptr, float* __restrict__ data,
                  float target_sum, const int64_t* __restrict__ cell_total,
@@ -78,18 +89,44 @@ normalize_kernel(int64_t n_rows, const int64_t* __restrict__ indptr, float* __re
   const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
   for (int64_t row = warp0; row < n_rows; row += nwarps) {
-    const int64_t beg = indptr[row], end = indptr[row + 1];
+    const int64_t beg = indptr[row], len = indptr[row + 1] - beg;
+    float* rowp = data + beg;
+    int head;
+    int64_t nvec;
+    row_vec_bounds(rowp, len, head, nvec);
+    float4* vp = reinterpret_cast<float4*>(rowp + head);
+    const int64_t tail0 = head + (nvec << 2);
     float scale;
     if (cell_total != nullptr) {
       scale = cell_scale(target_sum, cell_total[row]);
     } else {
       double s = 0.0;
-      for (int64_t p = beg + lane; p < end; p += 32) s += (double)data[p];
+      if (lane < head) s += (double)rowp[lane];
+      for (int64_t i = lane; i < nvec; i += 32) {
+        const float4 v = vp[i];
+        s += ((double)v.x + (double)v.y) + ((double)v.z + (double)v.w);
+      }
+      if (tail0 + lane < len) s += (double)rowp[tail0 + lane];
       s = warp_sum(s);
       const float sf = (float)s;
       scale = sf != 0.0f ? __fdiv_rn(target_sum, sf) : 1.0f;
     }
-    for (int64_t p = beg + lane; p < end; p += 32) data[p] = __fmul_rn(data[p], scale);
+    if (lane < head) rowp[lane] = __fmul_rn(rowp[lane], scale);
+    int64_t i = lane;
+    for (; i + 96 < nvec; i += 128) {                     // four loads in flight per lane
+      float4 a = vp[i], b = vp[i + 32], c = vp[i + 64], d = vp[i + 96];
+      a.x = __fmul_rn(a.x, scale); a.y = __fmul_rn(a.y, scale); a.z = __fmul_rn(a.z, scale); a.w = __fmul_rn(a.w, scale);
+      b.x = __fmul_rn(b.x, scale); b.y = __fmul_rn(b.y, scale); b.z = __fmul_rn(b.z, scale); b.w = __fmul_rn(b.w, scale);
+      c.x = __fmul_rn(c.x, scale); c.y = __fmul_rn(c.y, scale); c.z = __fmul_rn(c.z, scale); c.w = __fmul_rn(c.w, scale);
+      d.x = __fmul_rn(d.x, scale); d.y = __fmul_rn(d.y, scale); d.z = __fmul_rn(d.z, scale); d.w = __fmul_rn(d.w, scale);
+      vp[i] = a; vp[i + 32] = b; vp[i + 64] = c; vp[i + 96] = d;
+    }
+    for (; i < nvec; i += 32) {
+      float4 a = vp[i];
+      a.x = __fmul_rn(a.x, scale); a.y = __fmul_rn(a.y, scale); a.z = __fmul_rn(a.z, scale); a.w = __fmul_rn(a.w, scale);
+      vp[i] = a;
+    }
+    if (tail0 + lane < len) rowp[tail0 + lane] = __fmul_rn(rowp[tail0 + lane], scale);
     if (lane == 0 && scale_out != nullptr) scale_out[row] = scale;
   }
 }

@@ -60,13 +60,24 @@ def assert_hvg_matches(g, o, n_top, name, strict=True):
     np.testing.assert_allclose(gm, o["mean_t"], rtol=1e-12, atol=1e-300, err_msg=name)
     np.testing.assert_allclose(gd[ok], o["disp"][ok], rtol=1e-12, atol=1e-13, err_msg=name)
     gb = np_(g["bin"])
-    nb_diff = int(np.sum(gb != o["bin"]))
-    # libm ulp differences in log1p can move a gene sitting exactly on an edge
-    assert nb_diff <= (0 if strict else 2), f"{name}: {nb_diff} bin ids differ"
-    if nb_diff == 0:
-        assert np.array_equal(np.isnan(gz), np.isnan(o["disp_norm"])), f"{name}: z NaN pattern"
-        okz = ~np.isnan(o["disp_norm"])
-        np.testing.assert_allclose(gz[okz], o["disp_norm"][okz], rtol=1e-9, atol=1e-10, err_msg=name)
+    diff = np.nonzero(gb != o["bin"])[0]
+    # libm ulp differences in log1p can move a gene sitting exactly on a bin edge into the
+    # neighbouring bin.  Allowed (strict=False only) for at most 2 genes, and only when the gene
+    # really sits within 2 ulp of the edge it crossed; the bins such a gene left / entered have
+    # different members on the two sides, so their z-scores are not comparable -- every OTHER
+    # bin is still compared in full.
+    assert len(diff) <= (0 if strict else 2), f"{name}: {len(diff)} bin ids differ"
+    edges = o["edges"]
+    for j in diff:
+        assert abs(int(gb[j]) - int(o["bin"][j])) == 1, f"{name}: gene {j} moved by more than one bin"
+        e = edges[max(int(gb[j]), int(o["bin"][j]))]
+        assert abs(o["mean_t"][j] - e) <= 2 * np.spacing(abs(e)) and abs(gm[j] - e) <= 2 * np.spacing(abs(e)), \
+            f"{name}: gene {j} changed bin but is not on the edge"
+    affected = np.union1d(gb[diff], o["bin"][diff])
+    cmp = ~np.isin(o["bin"], affected)
+    assert np.array_equal(np.isnan(gz[cmp]), np.isnan(o["disp_norm"][cmp])), f"{name}: z NaN pattern"
+    okz = cmp & ~np.isnan(o["disp_norm"])
+    np.testing.assert_allclose(gz[okz], o["disp_norm"][okz], rtol=1e-9, atol=1e-10, err_msg=name)
     mask_g = np_(g["mask"]).astype(bool)
     mask_o = o["mask"].astype(bool)
     cnt = int(np_(g["count"])[0])
@@ -74,11 +85,12 @@ def assert_hvg_matches(g, o, n_top, name, strict=True):
     idx = np_(g["indices"])[:cnt]
     assert np.array_equal(idx, np.nonzero(mask_g)[0]), f"{name}: indices not the ascending mask positions"
     if not np.array_equal(mask_g, mask_o):
-        # identical except for ties at the cutoff (north_star; reading R13)
+        # identical except for ties at the cutoff (north_star; reading R13).  Genes of an affected
+        # bin (see above) carry z-scores of a different bin population and are left out.
         cutoff = o["cutoff"]
         band = 1e-9 * max(1.0, abs(cutoff))
-        diff = np.nonzero(mask_g != mask_o)[0]
-        zz = o["disp_norm"][diff]
+        d2 = np.nonzero((mask_g != mask_o) & cmp)[0]
+        zz = o["disp_norm"][d2]
         assert np.all(np.abs(zz - cutoff) <= band), f"{name}: HVG sets differ outside the tie band"
     valid = int((~np.isnan(o["disp_norm"])).sum())
     assert cnt >= min(n_top, valid)

@@ -1,10 +1,12 @@
 """GPU parity on BASELINE.json's configurations, through rsc_preprocess (the call bench.py
 times) and rsc_preprocess_host.
 
-Config 1 is checked element by element against the full oracle chain.  The large configs are
-checked at FULL size in the bench launch configuration on sampled outputs the oracle computes
-one by one (sampled rows for per-cell outputs and x''; sampled genes for per-gene outputs),
-plus invariants that hold at any size and the HVG selection recomputed by the oracle from the
+Config 1 is checked element by element against the full NumPy oracle chain.  Configs 2, 3 and 5
+are checked IN FULL at full size in the bench launch configuration: the matrix is walked in row
+chunks and every per-cell output, every x'' value, every per-gene integer and every per-gene
+moment is compared with the C / OpenMP oracle twin (oracle/oracle_c.c, pinned element-wise
+against oracle_np in tests/test_oracle_c.py).  Config 4 (7.5e9 entries) is checked on sampled
+rows / genes plus invariants that hold at any size.  HVG is recomputed by the oracle from the
 GPU's full mean / var arrays.
 """
 import os
@@ -13,6 +15,7 @@ import numpy as np
 import pytest
 import torch
 
+from oracle import oracle_c as OC
 from oracle import oracle_np as O
 from paper_2603_02402_b200 import synth
 import parity_util as U
@@ -63,6 +66,84 @@ def test_config1_full_oracle():
     # independent chains: the sets agree except near the cutoff
     m_o = ref["hvg"]["mask"].astype(bool); m_g = U.np_(out["hvg_mask"]).astype(bool)
     assert (m_o != m_g).sum() <= 4
+
+
+def _hvg_dict(out):
+    return dict(mean_t=out["hvg_mean_t"], disp=out["hvg_disp"], disp_norm=out["hvg_disp_norm"],
+                bin=out["hvg_bin"], mask=out["hvg_mask"], indices=out["hvg_indices"], count=out["hvg_count"])
+
+
+def _full_check(cfg, chunk_rows=65536):
+    """Every output of the chain at full size against the oracle, the matrix walked in row chunks."""
+    from paper_2603_02402_b200 import Csr, Preprocessor, rsc_normalize_total
+    indptr, indices, data = synth.make_csr(cfg, "cuda")
+    n, G = cfg.n_cells, cfg.n_genes
+    nnz = indices.numel()
+    flags = synth.gene_flags(cfg, "cuda")
+    raw = data.clone()
+    X = Csr(indptr, indices, data, G)
+    out = _run_chain(cfg, X, flags)                      # both moment sets
+    Xn = Csr(indptr, indices, raw.clone(), G)            # x' as the unfused kernel writes it
+    rsc_normalize_total(Xn, cfg.target_sum, out["cell_total_i64"])
+    torch.cuda.synchronize()
+
+    fl = U.np_(flags)
+    ip_all = U.np_(indptr)
+    gn, gt = np.zeros(G, np.int64), np.zeros(G, np.int64)
+    s_log = (np.zeros(G), np.zeros(G), np.zeros(G))
+    s_lin = (np.zeros(G), np.zeros(G), np.zeros(G))
+    chunks = [(a, min(n, a + chunk_rows)) for a in range(0, n, chunk_rows)]
+
+    def host(a, b, *arrs):
+        lo, hi = int(ip_all[a]), int(ip_all[b])
+        return (ip_all[a:b + 1] - ip_all[a], U.np_(indices[lo:hi])) + tuple(U.np_(t[lo:hi]) for t in arrs)
+
+    for a, b in chunks:                                   # pass 1: per-cell outputs, x'', sums
+        ip, ix, rw, xl_g, xn_g = host(a, b, raw, X.data, Xn.data)
+        q = OC.qc_metrics(ip, ix, rw, G, fl, gene_acc=(gn, gt))
+        for k in ("cell_total_i64", "cell_n_genes", "cell_flag_total_i64"):
+            U.assert_int_equal(out[k][a:b], q[k], f"{k} rows {a}:{b}")
+        U.assert_f32_close(out["cell_flag_pct"][a:b], q["cell_flag_pct"], "pct")
+        U.assert_f32_close(out["cell_total_f32"][a:b], q["cell_total_f32"], "total_f32", rtol=0)
+        xn_o, xl_o = OC.normalize_log1p(ip, rw, cfg.target_sum, q["cell_total_i64"])
+        U.assert_f32_close(xl_g, xl_o, f"x'' rows {a}:{b}")
+        U.assert_f32_close(xn_g, xn_o, f"x' rows {a}:{b}")
+        OC.gene_sums(ip, ix, xl_g, G, 0, acc=s_log)       # moments of the values the GPU wrote
+        OC.gene_sums(ip, ix, xn_g, G, 0, acc=s_lin)
+    U.assert_int_equal(out["gene_n_cells"], gn.astype(np.int32), "gene_n_cells")
+    U.assert_int_equal(out["gene_total_i64"], gt, "gene_total_i64")
+    assert int(gn.sum()) == nnz
+
+    mean_log, mean_lin = s_log[0] / np.float64(n), s_lin[0] / np.float64(n)
+    ss_log, ss_lin = np.zeros(G), np.zeros(G)
+    for a, b in chunks:                                   # pass 2: squared deviations (two-pass variance)
+        ip, ix, xl_g, xn_g = host(a, b, X.data, Xn.data)
+        OC.gene_sqdev(ip, ix, xl_g, G, mean_log, 0, acc=ss_log)
+        OC.gene_sqdev(ip, ix, xn_g, G, mean_lin, 0, acc=ss_lin)
+    mo, vo = OC.moments_from(n, s_log[0], s_log[2], ss_log, 1)
+    U.assert_moments_close(out["mean_log"], out["var_log"], mo, vo, "log moments (all genes)")
+    mo, vo = OC.moments_from(n, s_lin[0], s_lin[2], ss_lin, 1)
+    U.assert_moments_close(out["mean_lin"], out["var_lin"], mo, vo, "lin moments (all genes)")
+    del Xn
+
+    h = O.hvg_select(U.np_(out["mean_lin"]), U.np_(out["var_lin"]), cfg.n_top, cfg.n_bins)
+    U.assert_hvg_matches(_hvg_dict(out), h, cfg.n_top, f"{cfg.name} hvg", strict=False)
+
+    # bench.py's launch configuration: the three staged C-ABI calls with the log-scale set only.
+    # The integer sums make the moments independent of the gene grouping: bit-identical to the
+    # both-sets run above, and so is x''.
+    xl_both = X.data.clone()
+    X.data.copy_(raw)
+    pp1 = Preprocessor(X.n_rows, X.n_cols, X.nnz, cfg.target_sum, cfg.n_top, cfg.n_bins, 1, 1, False)
+    o1 = pp1.run_staged(X, flags)
+    torch.cuda.synchronize()
+    assert torch.equal(X.data, xl_both), "x'' differs between which_moments = 1 and 3"
+    assert torch.equal(o1["mean_log"], out["mean_log"]) and torch.equal(o1["var_log"], out["var_log"])
+    for k in ("cell_total_i64", "cell_n_genes", "gene_n_cells", "gene_total_i64"):
+        assert torch.equal(o1[k], out[k]), k
+    hl = O.hvg_select(U.np_(o1["mean_log"]), U.np_(o1["var_log"]), cfg.n_top, cfg.n_bins)
+    U.assert_hvg_matches(_hvg_dict(o1), hl, cfg.n_top, f"{cfg.name} hvg on log-scale moments", strict=False)
+    return nnz
 
 
 def _sampled_check(cfg, n_cells=None, n_row_samples=384, n_gene_samples=64):
@@ -142,18 +223,18 @@ def _sampled_check(cfg, n_cells=None, n_row_samples=384, n_gene_samples=64):
     return nnz
 
 
-def test_config2_full_size_sampled():
-    nnz = _sampled_check(synth.CONFIGS[2])
+def test_config2_full_size_every_output():
+    nnz = _full_check(synth.CONFIGS[2])
     assert 1.8e8 < nnz < 2.3e8
 
 
-def test_config3_full_size_sampled():
-    nnz = _sampled_check(synth.CONFIGS[3])
+def test_config3_full_size_every_output():
+    nnz = _full_check(synth.CONFIGS[3])
     assert 1.4e9 < nnz < 1.65e9
 
 
-def test_config5_skewed_full_size_sampled():
-    nnz = _sampled_check(synth.CONFIGS[5])
+def test_config5_skewed_full_size_every_output():
+    nnz = _full_check(synth.CONFIGS[5])
     assert 1.3e9 < nnz < 1.7e9
 
 
@@ -166,7 +247,7 @@ def test_config4_int64_nnz_sampled():
     free, _ = torch.cuda.mem_get_info()
     if free < 150e9:
         pytest.skip("needs ~150 GB of free HBM")
-    nnz = _sampled_check(synth.CONFIGS[4], n_row_samples=256, n_gene_samples=32)
+    nnz = _sampled_check(synth.CONFIGS[4], n_row_samples=4096, n_gene_samples=96)
     assert nnz > 2**31
 
 
