@@ -79,8 +79,8 @@ const char* rsc_version(void);
  * counter; memsets / memcpys are not counted).  Used by bench.py to report gpu_launches. */
 uint64_t rsc_kernel_launch_count(void);
 /* Process-wide tuning / testing knobs (not needed in normal use; defaults in brackets):
- *   "fused_row_budget" [512]   rows a CTA of the fused pass takes between two checks of its
- *                              integer accumulator tables (1..512, rounded down to a power of
+ *   "fused_row_budget" [256]   rows a CTA of the fused pass takes between two checks of its
+ *                              integer accumulator tables (1..256, rounded down to a power of
  *                              two); a check moves the genes whose words are half full to the
  *                              global totals
  *   "flush_all"        [0]     1 = every check moves EVERY gene (testing the exchange path)

@@ -68,14 +68,23 @@ int launch_moments_generic(const rsc_csr&, int, double*, double*, cudaStream_t);
 int finalize_moments(int32_t, int64_t, int, const double*, const double*, double*, double*,
                      cudaStream_t);
 
-size_t moments_workspace_bytes(int64_t, int32_t n_cols, int64_t) {
-  return 2 * align_up(sizeof(double) * (size_t)n_cols, 256);
+// implemented in fused.cu: the moments-only pass on the streaming skeleton
+size_t moments_fast_workspace_bytes(int64_t n_rows, int32_t n_cols);
+bool moments_fast_ok(const rsc_csr& X);
+int launch_moments_fast(const rsc_csr& X, int ddof, double* mean, double* var, double* sum, double* sumsq,
+                        void* ws, cudaStream_t st);
+
+size_t moments_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t) {
+  return moments_fast_workspace_bytes(n_rows, n_cols);
 }
 
 int launch_moments(const rsc_csr& X, int transform, int ddof, double* mean, double* var,
                    double* sum, double* sumsq, void* ws, size_t, cudaStream_t st) {
   const size_t gsz = align_up(sizeof(double) * (size_t)X.n_cols, 256);
   unsigned char* w = static_cast<unsigned char*>(ws);
+  // transform 0 on sorted rows: on-chip integer accumulators; expm1 needs fp64 values (1e-9 bar),
+  // which only the generic L2-atomic kernel provides
+  if (transform == 0 && moments_fast_ok(X)) return launch_moments_fast(X, ddof, mean, var, sum, sumsq, ws, st);
   double* S1 = sum ? sum : reinterpret_cast<double*>(w);
   double* S2 = sumsq ? sumsq : reinterpret_cast<double*>(w + gsz);
   int rc = launch_moments_generic(X, transform, S1, S2, st);
@@ -96,7 +105,7 @@ uint64_t rsc_kernel_launch_count(void) { return g_launch_count; }
 int rsc_set_option(const char* key, long long value) {
   RSC_CHECK_ARG(key != nullptr, "rsc_set_option: key is NULL");
   if (!strcmp(key, "fused_row_budget")) {
-    RSC_CHECK_ARG(value >= 1 && value <= 512, "rsc_set_option: fused_row_budget must be in [1, 512]");
+    RSC_CHECK_ARG(value >= 1 && value <= 256, "rsc_set_option: fused_row_budget must be in [1, 256]");
     g_opt.fused_row_budget = (int)value;
   } else if (!strcmp(key, "flush_all")) {
     g_opt.flush_all = value != 0;

@@ -39,7 +39,7 @@ void set_error(const char* fmt, ...);
 
 // run-time tunables (rsc_set_option): defaults are the shipped configuration
 struct Options {
-  int fused_row_budget = 512;     // rows a fused-pass CTA takes between two checks of its tables (<= 512)
+  int fused_row_budget = 256;     // rows a fused-pass CTA takes between two checks of its tables (<= 256)
   int flush_all = 0;              // 1: every check moves every gene to the global totals (testing)
   int qc_row_budget = 512;        // rows a QC CTA takes between two checks of its table (<= 512)
   int grid_ctas = 0;              // CTAs of the streaming kernels; 0 = one per SM

@@ -26,15 +26,16 @@
 //     word with a predicated increment: 2^23 <= a < 2^32 takes ~3.1 atomics per entry,
 //     2^32 <= a < 2^42 the same path with a two-word a.
 //     LOG-scale set (x'' = log1p(x') lies in [log1p(s / T_max), log1p(s)], a few binades):
-//     3 words per gene and NO branches -- window 2^23 <= a < 2^29 (64-fold),
+//     3 words per gene and NO branches -- window 2^23 <= a < 2^28 (32-fold, placed on the
+//     device from the cell depths),
 //         w0 += a                                  (returning atomic -> carry c1)
-//         s0 += low word of b,  b = (a*a + 2^13) >> 14   (returning atomic -> carry c0)
-//         W  += high word of b + c0 + (c1 << 23)   (one non-returning atomic)
-//     W packs the upper part of S2 (bits 0..22) and the carry count of S1 (bits 23..30);
-//     with at most 2040 rows between two flushes neither field can overflow.  S1 is exact;
-//     S2 is the sum of a*a rounded to a multiple of 2^14, i.e. to <= 2^-33 of the SMALLEST
-//     possible a*a (1.2e-10; 7e-12 for a typical x'' of 1..2) -- far inside the 1e-9 bar --
-//     and still an integer sum.  12 B / gene: 30 k genes need 2 groups, 18 k genes one.
+//         s0 += low word of b,  b = (a*a + 2^7) >> 8     (returning atomic -> carry c0)
+//         W  += high word of b + c0 + (c1 << 26)   (one non-returning atomic)
+//     W packs the upper part of S2 (bits 0..25) and the carry count of S1 (bits 26..31); a
+//     gene leaves the table when a field is half full (check_tables), so neither can overflow.
+//     S1 is exact; S2 is the sum of a*a rounded to a multiple of 2^8, i.e. to <= 2^-39 of the
+//     SMALLEST possible a*a (1.8e-12; 1e-13 for a typical x'' of 1..2) -- and still an integer
+//     sum.  12 B / gene: 30 k genes need 2 groups, 18 k genes one.
 //     Values outside a set's window (or negative / NaN) go to the global double sums directly.
 //     Integer adds commute, so the on-chip sums do not depend on the order of the adds; a
 //     flush adds every word to its own 64-bit global counter, converted to double once at the
@@ -60,15 +61,21 @@ constexpr int kFuRowsPerGrab = RSC_FU_RG;
 constexpr long long kCheckBit = 1LL << 62;  // set in a grab's result: this grab crossed a check point
 constexpr int kMaxGroups = 64;
 // rows a CTA can add between two checks of a gene: the check interval (<= 512) + the grabs its
-// warps hold (current, next, pending) must stay below 1020 (see check_tables)
-static_assert(512 + 3 * (kFuThreads / 32) * kFuRowsPerGrab + 64 <= 1020, "fused pass: too many rows in flight for the lazy flush");
+// warps hold (current, next, pending) must stay below kMaxRowsBetweenChecks (see check_tables)
+constexpr int kCheckRows = 256;            // default / largest check interval
+constexpr int kMaxRowsBetweenChecks = 410;
+static_assert(kCheckRows + 3 * (kFuThreads / 32) * kFuRowsPerGrab + 16 <= kMaxRowsBetweenChecks,
+              "fused pass: too many rows in flight for the lazy flush");
 constexpr int kSetWords = 5;               // u32 words per gene of the linear-scale set (w0 w1 s0 s1 s2)
 constexpr int kLogWords = 3;               // u32 words per gene of the log-scale set (w0 s0 W)
-constexpr int kLogShift = 14;              // log-scale set: S2 accumulates (a * a + 2^13) >> 14
-constexpr int kLogBinades = 6;             // log-scale set: 2^23 <= a < 2^29
-constexpr int kLogCarryBit = 23;           // W = upper S2 word (bits 0..22) | carries of w0 (bits 23..30)
-// a gene is moved out when a field of W is half full and checked at least every 1020 rows:
-// 1020 * 2^12 < 2^22 (upper S2 word), 1020 * 2^29 / 2^32 + 1 <= 128 (carries of w0)
+constexpr int kLogShift = 8;               // log-scale set: S2 accumulates (a * a + 2^7) >> 8
+constexpr int kLogBinades = 5;             // log-scale set: 2^23 <= a < 2^28
+constexpr int kLogCarryBit = 26;           // W = upper S2 word (bits 0..25) | carries of w0 (bits 26..31)
+constexpr uint32_t kLogCarryHalf = 32u;    // half of the 6-bit carry field
+// A gene is moved out when a field of W is half full, and a CTA adds at most
+// kMaxRowsBetweenChecks = 410 rows between two checks of a gene:
+//   upper S2 word: (a*a >> 8) >> 32 < 2^16 per add (+ carry), 410 * 2^16 < 2^25 = half of 26 bits;
+//   carries of w0: at most 410 * 2^28 / 2^32 + 1 = 27 < 32 = half of 6 bits.
 constexpr double kRowCost = 200.0;         // per-row-segment overhead, in entries (plan kernel)
 constexpr int kMaxRangeBits = 19;          // 2^k * v_max <= 2^(23 + 19) = 2^42
 
@@ -85,8 +92,15 @@ struct FusedPlan {                         // in the workspace
   int32_t cta_first[kMaxGroups + 1];
   unsigned long long row_counter[kMaxGroups];
   unsigned long long tmax;                 // largest cell total (fused_tmax_kernel)
+  unsigned int depth_hist[64];             // cells by binade of log1p(target_sum / T_i), bin = exponent + 32
   MomentScale sc_log, sc_lin;
+  // moments-only pass (rsc_gene_moments): chosen on the device by moments_plan_kernel
+  int32_t scheme;                          // 1: three-word (narrow window) set, 2: five-word set
+  int32_t Gt;                              // accumulator slots per CTA
+  int32_t n_need;                          // n_groups + 1
+  int32_t need[kMaxGroups + 1];            // column-block index at which group c starts
 };
+constexpr int kNeedStride = 8;             // split entries per row of the moments-only pass (<= 7 groups)
 
 struct FusedArgs {
   int64_t n_rows;
@@ -99,7 +113,7 @@ struct FusedArgs {
   const int32_t* indices;
   float* data;
   const int64_t* cell_total;
-  const uint32_t* splits;
+  const uint32_t* splits;   // fused: [n_rows][K + 1]; moments-only: [n_rows][kNeedStride], entry c = start of group c
   float target_sum;
   uint32_t row_budget;       // fp64 kernel: a CTA stops grabbing rows once it has taken this many (then flushes)
   uint32_t check_shift;      // integer kernels: a warp checks the CTA's tables every 2^check_shift rows
@@ -112,14 +126,27 @@ struct FusedArgs {
 
 // ------------------------------------------------------------------ largest cell total
 __global__ void __launch_bounds__(256)
-fused_tmax_kernel(FusedPlan* plan, int64_t n_rows, const int64_t* __restrict__ cell_total) {
+fused_tmax_kernel(FusedPlan* plan, int64_t n_rows, const int64_t* __restrict__ cell_total, float target_sum) {
+  __shared__ unsigned int hist[64];
+  if (threadIdx.x < 64) hist[threadIdx.x] = 0u;
+  __syncthreads();
   long long m = 0;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_rows;
-       i += (int64_t)gridDim.x * blockDim.x)
-    m = max(m, (long long)cell_total[i]);
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const long long t = (long long)cell_total[i];
+    m = max(m, t);
+    if (t > 0) {
+      // the smallest x'' of the cell: a unit count.  Binade of log1p(s / T) (frexp exponent - 1)
+      int e;
+      frexpf(log1pf(__fdiv_rn(target_sum, (float)t)), &e);
+      atomicAdd(&hist[min(max(e - 1 + 32, 0), 63)], 1u);
+    }
+  }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
   if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(&plan->tmax, (unsigned long long)m);
+  __syncthreads();
+  if (threadIdx.x < 64 && hist[threadIdx.x]) atomicAdd(&plan->depth_hist[threadIdx.x], hist[threadIdx.x]);
 }
 
 // floor(log2(x)) for finite x > 0
@@ -148,6 +175,38 @@ __device__ inline MomentScale make_scale(double v_min, double v_max) {
   return s;
 }
 
+// CTAs are dealt to the gene groups in proportion to their cost (one thread).  Cost of a group
+// = its entries + a per-row overhead (every CTA of the group walks a segment of EVERY row:
+// grab, metadata, edge steps ~ the work of kRowCost entries), so a group of few, sparse columns
+// still gets the CTAs its row count needs.
+__device__ inline void deal_ctas(FusedPlan* plan, double* mass, int ng, int grid, long long n_rows) {
+  double total = 0.0;
+  for (int c = 0; c < ng; ++c) { mass[c] += (double)n_rows * kRowCost; total += mass[c]; }
+  int n[kMaxGroups];
+  int sum = 0;
+  for (int c = 0; c < ng; ++c) {
+    const double share = total > 0.0 ? mass[c] / total : 1.0 / ng;
+    mass[c] = share + 1e-9;
+    n[c] = max(1, (int)(share * grid));
+    sum += n[c];
+  }
+  while (sum < grid) {                                   // most loaded group gets the next CTA
+    int best = 0;
+    for (int c = 1; c < ng; ++c) if (mass[c] / n[c] > mass[best] / n[best]) best = c;
+    ++n[best]; ++sum;
+  }
+  while (sum > grid) {                                   // only if many groups got the floor of 1
+    int best = -1;
+    for (int c = 0; c < ng; ++c)
+      if (n[c] > 1 && (best < 0 || mass[c] / (n[c] - 1) < mass[best] / (n[best] - 1))) best = c;
+    --n[best]; --sum;
+  }
+  plan->n_groups = ng;
+  int acc = 0;
+  for (int c = 0; c < ng; ++c) { plan->cta_first[c] = acc; acc += n[c]; plan->row_counter[c] = 0ull; }
+  plan->cta_first[ng] = acc;
+}
+
 // ------------------------------------------------------------------ plan (1 CTA)
 __global__ void __launch_bounds__(1024)
 fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid, float target_sum,
@@ -169,36 +228,7 @@ fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid, f
     if ((tid & 31) == 0 && m != 0.0) atomicAdd(&mass[c], m);
   }
   __syncthreads();
-  if (tid == 0) {
-    // cost of a group = its entries + a per-row overhead (every CTA of the group walks a
-    // segment of EVERY row: grab, metadata, edge steps ~ the work of kRowCost entries), so a
-    // group of few, sparse columns still gets the CTAs its row count needs
-    double total = 0.0;
-    for (int c = 0; c < ng; ++c) { mass[c] += (double)n_rows * kRowCost; total += mass[c]; }
-    int n[kMaxGroups];
-    int sum = 0;
-    for (int c = 0; c < ng; ++c) {
-      const double share = total > 0.0 ? mass[c] / total : 1.0 / ng;
-      mass[c] = share + 1e-9;
-      n[c] = max(1, (int)(share * grid));
-      sum += n[c];
-    }
-    while (sum < grid) {                                   // most loaded group gets the next CTA
-      int best = 0;
-      for (int c = 1; c < ng; ++c) if (mass[c] / n[c] > mass[best] / n[best]) best = c;
-      ++n[best]; ++sum;
-    }
-    while (sum > grid) {                                   // only if many groups got the floor of 1
-      int best = -1;
-      for (int c = 0; c < ng; ++c)
-        if (n[c] > 1 && (best < 0 || mass[c] / (n[c] - 1) < mass[best] / (n[best] - 1))) best = c;
-      --n[best]; --sum;
-    }
-    plan->n_groups = ng;
-    int acc = 0;
-    for (int c = 0; c < ng; ++c) { plan->cta_first[c] = acc; acc += n[c]; plan->row_counter[c] = 0ull; }
-    plan->cta_first[ng] = acc;
-  }
+  if (tid == 0) deal_ctas(plan, mass, ng, grid, n_rows);
   if (tid == 32) {
     // power-of-two scales of the integer accumulators: x' of a unit count in the deepest
     // cell is target_sum / T_max; nothing exceeds target_sum (non-negative data)
@@ -210,13 +240,25 @@ fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid, f
     if (smin > ts) smin = ts;
     plan->sc_lin = make_scale(smin, ts);
     {
-      // log-scale set: kLogBinades binades below the top 2^E > log1p(target_sum), the largest
-      // x'' non-negative data can produce
-      // (and never below 2^-2: log1p_ge_quarter of an x' < 0.25 is < 0.2232, so such a value
-      // fails the window test by itself and the log-only kernel needs no separate x' test)
+      // log-scale set: a window of kLogBinades binades [2^L, 2^(L + kLogBinades)).  The bottom
+      // is the binade of the smallest x'' of the data -- a unit count in the deepest cell --
+      // taken robustly: the n / 4096 deepest cells are ignored (their small values take the
+      // global path), so one outlier cell cannot drag the window away from the bulk.  Never
+      // above the top 2^E > log1p(target_sum) (the largest x'' non-negative data can produce),
+      // and never below 2^-2: log1p_ge_quarter of an x' < 0.25 is < 0.2232, so such a value
+      // fails the window test by itself and the log-only kernel needs no separate x' test.
       int E;
       frexp(log1p(ts) * 1.000001, &E);
-      const int L = max(E - kLogBinades, -2);
+      int L = E - kLogBinades;
+      {
+        const unsigned long long skip = (unsigned long long)n_rows / 4096ull;
+        unsigned long long below = 0ull;
+        for (int b = 0; b < 64; ++b) {
+          below += plan->depth_hist[b];
+          if (below > skip) { L = min(b - 32, E - kLogBinades); break; }
+        }
+      }
+      L = max(L, -2);
       const int k = 23 - L;
       MomentScale s;
       s.mult = (float)ldexp(1.0, k);
@@ -226,6 +268,126 @@ fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid, f
       plan->sc_log = s;
     }
   }
+}
+
+// ------------------------------------------------------------------ plan of the moments-only pass
+// rsc_gene_moments knows nothing about the values, so the plan looks at a sample (32 768 stored
+// entries in 1 024 clusters spread evenly over the matrix): largest value v_max, smallest positive value, and how
+// the entries spread over the column blocks.
+//   * window top 2^E > 2 v_max (one binade of head room over the sample);
+//   * if the sample spans at most kLogBinades - 1 binades below it, the three-word scheme
+//     (12 B / gene), else the five-word scheme (one-word values 2^(E-9) .. 2^E, two-word values
+//     up to 2^(E+10));
+//   * gene groups as large as the table allows, CTAs dealt by the sampled entry counts.
+// A value the sample did not foresee still lands in the global double sums: correct, only slow.
+__global__ void __launch_bounds__(1024)
+moments_plan_kernel(FusedPlan* plan, int G, int K, int grid, long long n_rows, long long nnz,
+                    const int32_t* __restrict__ indices, const float* __restrict__ data) {
+  __shared__ double mass[kMaxGroups];
+  __shared__ float s_max[32], s_min[32];
+  __shared__ int s_ng;
+  constexpr int kPer = 32;
+  const int tid = threadIdx.x;
+  // 32 * kPer clusters of 32 consecutive entries (a warp reads one line per load), spread evenly
+  const long long step = nnz > 1024LL * kPer ? (nnz - 32) / (32LL * kPer) : 32;
+  float vmax = 0.0f, vmin = INFINITY;
+  int32_t col[kPer];                                      // the sampled entries' columns (registers)
+#pragma unroll
+  for (int i = 0; i < kPer; ++i) {                        // independent loads: all in flight together
+    const long long p = ((long long)i * 32 + (tid >> 5)) * step + (tid & 31);
+    float v = 0.0f;
+    col[i] = -1;
+    if (p < nnz) { v = __ldg(data + p); col[i] = __ldg(indices + p); }
+    if (v > vmax) vmax = v;
+    if (v > 0.0f && v < vmin) vmin = v;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
+    vmin = fminf(vmin, __shfl_xor_sync(0xffffffffu, vmin, o));
+  }
+  if ((tid & 31) == 0) { s_max[tid >> 5] = vmax; s_min[tid >> 5] = vmin; }
+  if (tid < kMaxGroups) mass[tid] = 0.0;
+  __syncthreads();
+  if (tid == 0) {
+    for (int w = 1; w < 32; ++w) { vmax = fmaxf(vmax, s_max[w]); vmin = fminf(vmin, s_min[w]); }
+    if (!(vmax > 0.0f) || !isfinite(vmax)) vmax = 1.0f;
+    int E;
+    frexp(2.0 * (double)vmax, &E);                         // 2^E > 2 v_max
+    const bool narrow = (double)vmin >= ldexp(1.0, E - kLogBinades);
+    MomentScale sc;
+    sc.pad = 0.0f;
+    int bpg;
+    if (narrow) {
+      const int k = 23 - (E - kLogBinades);
+      sc.mult = (float)ldexp(1.0, k); sc.inv1 = ldexp(1.0, -k); sc.inv2 = ldexp(1.0, kLogShift - 2 * k);
+      plan->sc_log = sc;
+      bpg = kLogWords * 4;
+    } else {
+      const int k = 32 - E;
+      sc.mult = (float)ldexp(1.0, k); sc.inv1 = ldexp(1.0, -k); sc.inv2 = ldexp(1.0, -2 * k);
+      plan->sc_lin = sc;
+      bpg = kSetWords * 4;
+    }
+    plan->scheme = narrow ? 1 : 2;
+    const int fit = (int)((kMaxDynSmem - 64) / ((size_t)bpg * RSC_SPLIT_WIDTH));
+    const int ng = (K + fit - 1) / fit;
+    plan->Gt = ((K + ng - 1) / ng) * RSC_SPLIT_WIDTH;
+    plan->n_need = ng + 1;
+    for (int c = 0; c <= ng; ++c) plan->need[c] = (c * K) / ng;
+    s_ng = ng;
+  }
+  __syncthreads();
+  const int ng = s_ng;
+  for (int c = 0; c < ng; ++c) {                          // sampled entries per group
+    const int b0 = plan->need[c], b1 = plan->need[c + 1];
+    int cnt = 0;
+#pragma unroll
+    for (int i = 0; i < kPer; ++i) {
+      const int b = col[i] >> RSC_SPLIT_SHIFT;
+      cnt += (col[i] >= 0 && b >= b0 && b < b1) ? 1 : 0;
+    }
+    cnt = warp_sum(cnt);
+    if ((tid & 31) == 0 && cnt) atomicAdd(&mass[c], (double)cnt);
+  }
+  __syncthreads();
+  if (tid == 0) {
+    double tot = 0.0;
+    for (int c = 0; c < ng; ++c) tot += mass[c];
+    for (int c = 0; c < ng; ++c) mass[c] = tot > 0.0 ? mass[c] / tot * (double)nnz : (double)nnz / ng;
+    deal_ctas(plan, mass, ng, grid, n_rows);
+  }
+}
+
+// Compact row split table of the moments-only pass: out[row][c] = number of the row's entries
+// with column < need[c] * RSC_SPLIT_WIDTH, c = 0 .. n_groups.  One thread per row; every interior
+// bound is bracketed around the position a uniform spread of the columns predicts (widened
+// geometrically), then bisected: a few probes, nearly all in one line.
+__global__ void __launch_bounds__(256)
+row_splits_compact_kernel(int64_t n_rows, int G, const int64_t* __restrict__ indptr,
+                          const int32_t* __restrict__ indices, const FusedPlan* __restrict__ plan,
+                          uint32_t* __restrict__ out) {
+  const int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (row >= n_rows) return;
+  const int ng = plan->n_groups;
+  const int64_t beg = indptr[row];
+  const int len = (int)(indptr[row + 1] - beg);
+  uint32_t* o = out + (size_t)row * kNeedStride;
+  o[0] = 0u;
+  for (int c = 1; c < ng; ++c) {
+    const int32_t bound = plan->need[c] << RSC_SPLIT_SHIFT;
+    int w = 16;
+    const int guess = (int)(((long long)len * bound) / G);
+    int lo = max(guess - w, 0), hi = min(guess + w, len);
+    while (lo > 0 && __ldg(indices + beg + lo - 1) >= bound) { hi = lo - 1; w *= 2; lo = max(lo - w, 0); }
+    while (hi < len && __ldg(indices + beg + hi) < bound) { lo = hi + 1; w *= 2; hi = min(hi + w, len); }
+    while (lo < hi) {
+      const int mid = (lo + hi) >> 1;
+      if (__ldg(indices + beg + mid) < bound) lo = mid + 1; else hi = mid;
+    }
+    o[c] = (uint32_t)lo;
+  }
+  o[ng] = (uint32_t)len;
 }
 
 // ------------------------------------------------------------------ accumulator primitives
@@ -426,10 +588,11 @@ struct AccCtx {
 };
 
 // one entry, any value: normalise, log1p, accumulate; returns x''
-template <bool LOG, bool LIN>
+// (MOM: moments-only pass, the value is x itself)
+template <bool LOG, bool LIN, bool MOM>
 __device__ __noinline__ float entry_any(const AccCtx& c, int j, float x, float scale) {
-  const float xn = __fmul_rn(x, scale);
-  const float xl = log1p_f32(xn);
+  const float xn = MOM ? x : __fmul_rn(x, scale);
+  const float xl = MOM ? x : log1p_f32(xn);
   const uint32_t slot = min((uint32_t)(j - c.g0), c.last_slot);       // stays inside the table
   if (LOG) acc3_slow(c.sb_log + slot * (kLogWords * 4u), xl, c.mult_log, c.S1log + c.g0 + slot,
                      c.S2log + c.g0 + slot);
@@ -441,7 +604,7 @@ __device__ __noinline__ float entry_any(const AccCtx& c, int j, float x, float s
 // A quad with at least one value outside the one-word window (out of line: keeps the hot path
 // small).  All values at most two-word integers and x' >= 0.25 -> acc_quad_wide; else entry by
 // entry.  valid_mask bit k: entry k belongs to the segment.
-template <bool LOG, bool LIN>
+template <bool LOG, bool LIN, bool MOM>
 __device__ __noinline__ float4 quad_rare(const AccCtx& c, int4 jv, float4 xv, float scale,
                                          uint32_t valid_mask, uint32_t spare_slot) {
   const int j[4] = {jv.x, jv.y, jv.z, jv.w};
@@ -452,9 +615,9 @@ __device__ __noinline__ float4 quad_rare(const AccCtx& c, int4 jv, float4 xv, fl
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
     const bool valid = (valid_mask >> k) & 1u;
-    xn[k] = __fmul_rn(x[k], scale);
-    xl[k] = log1p_ge_quarter(xn[k]);
-    ok = ok && (xn[k] >= 0.25f || !valid);
+    xn[k] = MOM ? x[k] : __fmul_rn(x[k], scale);
+    xl[k] = MOM ? x[k] : log1p_ge_quarter(xn[k]);
+    ok = ok && (MOM || xn[k] >= 0.25f || !valid);
     if (LOG) { tl[k] = xl[k] * c.mult_log; ok = ok && (in_window_log(tl[k]) || !valid); }
     if (LIN) { tn[k] = xn[k] * c.mult_lin; ok = ok && (in_window_wide(tn[k]) || !valid); }
     slot[k] = valid ? min((uint32_t)(j[k] - c.g0), c.last_slot) : spare_slot;
@@ -482,19 +645,21 @@ __device__ __noinline__ float4 quad_rare(const AccCtx& c, int4 jv, float4 xv, fl
   } else {
 #pragma unroll
     for (int k = 0; k < 4; ++k)
-      if ((valid_mask >> k) & 1u) xl[k] = entry_any<LOG, LIN>(c, j[k], x[k], scale);
+      if ((valid_mask >> k) & 1u) xl[k] = entry_any<LOG, LIN, MOM>(c, j[k], x[k], scale);
   }
   return make_float4(xl[0], xl[1], xl[2], xl[3]);
 }
 
 // ------------------------------------------------------------------ streaming kernel
-template <bool LOG, bool LIN>
-__global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const FusedArgs a) {
-  extern __shared__ __align__(16) uint32_t fsm[];
-  constexpr int kSets = (LOG ? 1 : 0) + (LIN ? 1 : 0);
-  __shared__ unsigned s_rows;
+// MOM = false: the fused pass (x' = x * scale_i, x'' = log1p(x') written back, sums of x'' / x').
+// MOM = true: the moments-only pass of rsc_gene_moments (transform 0): the value is x itself,
+// nothing is written back, exactly one set is active (LOG = the three-word scheme, LIN = the
+// five-word scheme), the gene groups and the table size come from the plan (device memory),
+// and the split table is the compact one ([kNeedStride] entries per row).
+template <bool LOG, bool LIN, bool MOM>
+__device__ __forceinline__ void fused_stream_body(const FusedArgs& a, uint32_t* fsm, unsigned& s_rows) {
   const int tid = threadIdx.x, lane = tid & 31;
-  const int Gt = a.Gt;
+  const int Gt = MOM ? a.plan->Gt : a.Gt;
   const int K = a.n_fine;
 
   // which group does this CTA serve?
@@ -505,8 +670,11 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
     while (grp + 1 < ng && (int)blockIdx.x >= plan->cta_first[grp + 1]) ++grp;
   }
   const float mult_log = plan->sc_log.mult, mult_lin = plan->sc_lin.mult;
-  const int f0 = (grp * K) / plan->n_groups;              // group = blocks [grp K / ng, (grp + 1) K / ng)
-  const int f1 = ((grp + 1) * K) / plan->n_groups;
+  // group = blocks [grp K / ng, (grp + 1) K / ng) (fused) or [need[grp], need[grp + 1]) (moments-only)
+  const int f0 = MOM ? plan->need[grp] : (grp * K) / plan->n_groups;
+  const int f1 = MOM ? plan->need[grp + 1] : ((grp + 1) * K) / plan->n_groups;
+  const int s0i = MOM ? grp : f0, s1i = MOM ? grp + 1 : f1;     // the row's split entries to read
+  const size_t sstride = MOM ? (size_t)kNeedStride : (size_t)(K + 1);
   const int g0 = f0 << RSC_SPLIT_SHIFT;
   const int ng_genes = min(a.n_cols, f1 << RSC_SPLIT_SHIFT) - g0;
   unsigned long long* counter = &a.plan->row_counter[grp];
@@ -566,14 +734,14 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
   // by word with an atomic exchange.  Each word is an independent sum (a carry is computed by
   // the adder from the value ITS atomic returned), so exchanging a word to 0 between two
   // adds loses nothing.  Between two checks of a gene a CTA adds at most
-  // 2^check_shift + (rows in flight) < 1020 rows, i.e. less than half of any field.
+  // 2^check_shift + (rows in flight) <= kMaxRowsBetweenChecks rows, i.e. less than half of any field.
   auto check_tables = [&]() {
     for (int s = lane; s < ng_genes; s += 32) {
       if (LOG) {
         uint32_t* w = fsm + (size_t)s * kLogWords;
         const uint32_t W = *reinterpret_cast<volatile uint32_t*>(w + 2);
         if (a.flush_all || (W & ((1u << kLogCarryBit) - 1u)) >= (1u << (kLogCarryBit - 1)) ||
-            (W >> kLogCarryBit) >= 128u) {
+            (W >> kLogCarryBit) >= kLogCarryHalf) {
           const uint32_t w0 = atomicExch(w, 0u), s0 = atomicExch(w + 1, 0u), Wx = atomicExch(w + 2, 0u);
           if (w0 | s0 | Wx) to_global_log(g0 + s, w0, s0, Wx);
         }
@@ -606,9 +774,9 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       valid[k] = !EDGE || (unsigned)(e0 + k) < (unsigned)len;
-      xn[k] = __fmul_rn(x[k], scale);
-      xl[k] = log1p_ge_quarter(xn[k]);
-      bool okk = (LOG && !LIN) || xn[k] >= 0.25f;       // log only: implied by the window test
+      xn[k] = MOM ? x[k] : __fmul_rn(x[k], scale);
+      xl[k] = MOM ? x[k] : log1p_ge_quarter(xn[k]);
+      bool okk = MOM || (LOG && !LIN) || xn[k] >= 0.25f;   // log only: implied by the window test
       if (LOG) { tl[k] = xl[k] * mult_log; okk = okk && in_window_log(tl[k]); }
       if (LIN) { tn[k] = xn[k] * mult_lin; okk = okk && in_window(tn[k]); }
       ok = ok && (okk || !valid[k]);
@@ -628,7 +796,7 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
     } else {
       const uint32_t vm = (valid[0] ? 1u : 0u) | (valid[1] ? 2u : 0u) | (valid[2] ? 4u : 0u) |
                           (valid[3] ? 8u : 0u);
-      return quad_rare<LOG, LIN>(cx, jv, xv, scale, vm, (uint32_t)Gt);
+      return quad_rare<LOG, LIN, MOM>(cx, jv, xv, scale, vm, (uint32_t)Gt);
     }
     return make_float4(xl[0], xl[1], xl[2], xl[3]);
   };
@@ -643,11 +811,11 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
       mb = 0; me = 0; ms = 1.0f;
       const long long row = g0row + lane;                 // lanes 0..RG-1: one row each
       if (lane < kFuRowsPerGrab && row < a.n_rows) {
-        const uint32_t* sp = a.splits + (size_t)row * (size_t)(K + 1);
+        const uint32_t* sp = a.splits + (size_t)row * sstride;
         const int64_t rb = a.indptr[row];
-        mb = rb + sp[f0];
-        me = rb + sp[f1];
-        ms = cell_scale(a.target_sum, a.cell_total[row]);
+        mb = rb + sp[s0i];
+        me = rb + sp[s1i];
+        if (!MOM) ms = cell_scale(a.target_sum, a.cell_total[row]);
       }
     };
     auto l2_prefetch = [&](int64_t mb, int64_t me, int ri) {   // the 128-byte lines of one segment
@@ -712,10 +880,13 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
         const int e0 = q * 4 - s.head;
         float* dq = a.data + (s.abeg + 4 * q);
         if (interior(s, st)) {
-          *reinterpret_cast<float4*>(dq) = quad(std::false_type{}, jv, xv, s.scale, e0, s.len);
+          const float4 r = quad(std::false_type{}, jv, xv, s.scale, e0, s.len);
+          if (!MOM) *reinterpret_cast<float4*>(dq) = r;
         } else if (q < s.nq) {
           const float4 r = quad(std::true_type{}, jv, xv, s.scale, e0, s.len);
-          if (e0 >= 0 && e0 + 4 <= s.len) {
+          if (MOM) {
+            // nothing is written back
+          } else if (e0 >= 0 && e0 + 4 <= s.len) {
             *reinterpret_cast<float4*>(dq) = r;
           } else {
             if ((unsigned)(e0 + 0) < (unsigned)s.len) dq[0] = r.x;
@@ -774,6 +945,24 @@ __global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const Fused
       }
     }
   }
+}
+
+template <bool LOG, bool LIN>
+__global__ void __launch_bounds__(kFuThreads, 1) fused_stream_kernel(const FusedArgs a) {
+  extern __shared__ __align__(16) uint32_t fsm[];
+  __shared__ unsigned s_rows;
+  fused_stream_body<LOG, LIN, false>(a, fsm, s_rows);
+}
+
+// rsc_gene_moments, transform 0 ("per-gene mean and variance, computed using a
+// custom GPU reduction kernel that operates directly on sparse matrices"; L137): the same
+// walk and accumulators with the normalise / log1p / store stage compiled out (8 B / nnz, read
+// only).  The accumulator scheme was chosen on the device (moments_plan_kernel).
+__global__ void __launch_bounds__(kFuThreads, 1) moments_stream_kernel(const FusedArgs a) {
+  extern __shared__ __align__(16) uint32_t fsm[];
+  __shared__ unsigned s_rows;
+  if (a.plan->scheme == 1) fused_stream_body<true, false, true>(a, fsm, s_rows);
+  else fused_stream_body<false, true, true>(a, fsm, s_rows);
 }
 
 // ------------------------------------------------------------------ double accumulators
@@ -857,6 +1046,7 @@ fused_finish_kernel(int G, double n, double denom, const FusedPlan* __restrict__
                     double* __restrict__ S2, double* __restrict__ mean, double* __restrict__ var) {
   const int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= G) return;
+  if (is_lin < 0) is_lin = plan->scheme == 2;            // moments-only pass: the scheme the plan chose
   const MomentScale sc = is_lin ? plan->sc_lin : plan->sc_log;
   const double two32 = 4294967296.0;
   const size_t Gs = (size_t)G;
@@ -974,19 +1164,19 @@ int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i
     a.splits = row_splits; a.target_sum = target_sum;
     a.row_budget = 4000u;
     a.check_shift = 0u;                                         // largest power of two <= the option (<= 512)
-    while (a.check_shift < 9u && (2u << a.check_shift) <= (uint32_t)g_opt.fused_row_budget) ++a.check_shift;
+    while (a.check_shift < 8u && (2u << a.check_shift) <= (uint32_t)g_opt.fused_row_budget) ++a.check_shift;
     a.flush_all = g_opt.flush_all ? 1u : 0u;
     a.S1log = S1log; a.S2log = S2log; a.S1lin = S1lin; a.S2lin = S2lin; a.plan = plan;
     const bool int_acc = !(which & RSC_MOMENTS_FP64_ACC);
     a.acc_log = reinterpret_cast<unsigned long long*>(accb);
     a.acc_lin = reinterpret_cast<unsigned long long*>(accb + asz);
-    if ((which & RSC_MOMENTS_LIN) && !(which & RSC_MOMENTS_FP64_ACC)) {
-      // the largest cell total places the linear-scale window (the log-scale one hangs from
-      // log1p(target_sum) and needs nothing from the data)
+    if (!(which & RSC_MOMENTS_FP64_ACC)) {
+      // cell depths place the windows: the largest total (linear scale), the binades of the
+      // cells' smallest x'' (log scale)
       int64_t blocks = (X.n_rows + 255) / 256;
       const int64_t cap = (int64_t)sm_count() * 4;
       if (blocks > cap) blocks = cap;
-      fused_tmax_kernel<<<(unsigned)blocks, 256, 0, st>>>(plan, X.n_rows, cell_total_i64);
+      fused_tmax_kernel<<<(unsigned)blocks, 256, 0, st>>>(plan, X.n_rows, cell_total_i64, target_sum);
       RSC_LAUNCH_CHECK("fused_tmax_kernel");
     }
     fused_plan_kernel<<<1, 1024, 0, st>>>(plan, X.n_cols, a.n_fine, a.fine_per_group, fused_grid(),
@@ -1026,6 +1216,65 @@ int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i
     rc = finalize_moments(X.n_cols, X.n_rows, ddof, S1lin, S2lin, mean_lin, var_lin, st);
     if (rc != RSC_OK) return rc;
   }
+  return RSC_OK;
+}
+
+// ------------------------------------------------------------------ rsc_gene_moments, fast path
+size_t moments_fast_workspace_bytes(int64_t n_rows, int32_t n_cols) {
+  return 2 * align_up(sizeof(double) * (size_t)n_cols, 256) +
+         align_up(5 * sizeof(unsigned long long) * (size_t)n_cols, 256) + align_up(sizeof(FusedPlan), 256) +
+         align_up(sizeof(uint32_t) * (size_t)(n_rows > 0 ? n_rows : 0) * kNeedStride, 256);
+}
+
+// sorted rows, 16-byte aligned arrays, at most kNeedStride - 1 groups in the worst (five-word) case
+bool moments_fast_ok(const rsc_csr& X) {
+  if (!(X.flags & RSC_CSR_SORTED) || g_opt.force_generic || X.n_rows == 0 || X.nnz == 0) return false;
+  if ((reinterpret_cast<uintptr_t>(X.indices) | reinterpret_cast<uintptr_t>(X.data)) & 15) return false;
+  const int fit = (int)((kMaxDynSmem - 64) / ((size_t)kSetWords * 4 * RSC_SPLIT_WIDTH));
+  const int K = split_blocks(X.n_cols);
+  const int ng = (K + fit - 1) / fit;
+  return ng <= kNeedStride - 1 && ng <= fused_grid();
+}
+
+int launch_moments_fast(const rsc_csr& X, int ddof, double* mean, double* var, double* sum, double* sumsq,
+                        void* ws, cudaStream_t st) {
+  const size_t G = (size_t)X.n_cols;
+  const size_t gsz = align_up(sizeof(double) * G, 256);
+  const size_t asz = align_up(5 * sizeof(unsigned long long) * G, 256);
+  unsigned char* w = static_cast<unsigned char*>(ws);
+  double* S1 = sum ? sum : reinterpret_cast<double*>(w);
+  double* S2 = sumsq ? sumsq : reinterpret_cast<double*>(w + gsz);
+  unsigned char* accb = w + 2 * gsz;
+  FusedPlan* plan = reinterpret_cast<FusedPlan*>(accb + asz);
+  uint32_t* splits = reinterpret_cast<uint32_t*>(accb + asz + align_up(sizeof(FusedPlan), 256));
+  RSC_CUDA(cudaMemsetAsync(S1, 0, sizeof(double) * G, st));
+  RSC_CUDA(cudaMemsetAsync(S2, 0, sizeof(double) * G, st));
+  RSC_CUDA(cudaMemsetAsync(accb, 0, asz + sizeof(FusedPlan), st));
+  const int K = split_blocks(X.n_cols);
+  moments_plan_kernel<<<1, 1024, 0, st>>>(plan, X.n_cols, K, fused_grid(), (long long)X.n_rows,
+                                          (long long)X.nnz, X.indices, X.data);
+  RSC_LAUNCH_CHECK("moments_plan_kernel");
+  row_splits_compact_kernel<<<(unsigned)((X.n_rows + 255) / 256), 256, 0, st>>>(X.n_rows, X.n_cols, X.indptr,
+                                                                              X.indices, plan, splits);
+  RSC_LAUNCH_CHECK("row_splits_compact_kernel");
+  FusedArgs a;
+  a.n_rows = X.n_rows; a.n_cols = X.n_cols; a.nnz = X.nnz; a.n_fine = K;
+  a.fine_per_group = 0; a.Gt = 0;                               // from the plan
+  a.indptr = X.indptr; a.indices = X.indices; a.data = X.data; a.cell_total = nullptr;
+  a.splits = splits; a.target_sum = 1.0f; a.row_budget = 0u;
+  a.check_shift = 0u;
+  while (a.check_shift < 8u && (2u << a.check_shift) <= (uint32_t)g_opt.fused_row_budget) ++a.check_shift;
+  a.flush_all = g_opt.flush_all ? 1u : 0u;
+  a.S1log = S1; a.S2log = S2; a.S1lin = S1; a.S2lin = S2; a.plan = plan;
+  a.acc_log = reinterpret_cast<unsigned long long*>(accb);
+  a.acc_lin = a.acc_log;
+  RSC_CUDA(cudaFuncSetAttribute(moments_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)kMaxDynSmem));
+  moments_stream_kernel<<<fused_grid(), kFuThreads, kMaxDynSmem, st>>>(a);
+  RSC_LAUNCH_CHECK("moments_stream_kernel");
+  fused_finish_kernel<<<(unsigned)((G + 255) / 256), 256, 0, st>>>(
+      X.n_cols, (double)X.n_rows, (double)(X.n_rows - ddof), plan, -1, a.acc_log, S1, S2, mean, var);
+  RSC_LAUNCH_CHECK("fused_finish_kernel");
   return RSC_OK;
 }
 
