@@ -129,6 +129,38 @@ __device__ __forceinline__ T warp_sum(T v) {
   return v;
 }
 
+// Streaming accesses.  The matrix is read once: a line that was used is dead, a line the
+// look-ahead has just fetched is not.  Demand loads / stores therefore carry an L2 evict_first
+// policy (createpolicy) so that used lines leave the L2 before prefetched ones do.
+__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ int4 ldg_stream_i4(const void* p, uint64_t pol) {
+  int4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.s32 {%0,%1,%2,%3}, [%4], %5;"
+               : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p), "l"(pol));
+  return v;
+}
+__device__ __forceinline__ float4 ldg_stream_f4(const void* p, uint64_t pol) {
+  float4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(pol));
+  return v;
+}
+// (not .nc: the fused pass rewrites the array it reads)
+__device__ __forceinline__ float4 ld_stream_f4(const void* p, uint64_t pol) {
+  float4 v;
+  asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(pol) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_stream_f4(void* p, float4 v, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1,%2,%3,%4}, %5;"
+               :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "l"(pol) : "memory");
+}
+
 // x'' = log(1 + x') in float32, shared by rsc_log1p and the fused pass so that
 // both write bit-identical values.  x >= 0.25: MUFU lg2 of the rounded 1 + x (absolute error
 // <= 2^-22 * ln 2 + 2^-24, i.e. <= 1e-6 relative there, ~1 ulp for typical x'' of 1..3);

@@ -35,7 +35,10 @@ constexpr int kQcRowsPerGrab = RSC_QC_RG;
 #ifndef RSC_QC_AHEAD
 #define RSC_QC_AHEAD 4
 #endif
-constexpr int kQcAhead = RSC_QC_AHEAD;                  // L2 look-ahead of a warp, in steps of 128 entries
+constexpr int kQcAhead = RSC_QC_AHEAD;
+#ifndef RSC_QC_EVICT
+#define RSC_QC_EVICT 0        // bit 0: demand loads carry L2 evict_first; bit 1: look-ahead prefetches carry evict_last
+#endif                  // L2 look-ahead of a warp, in steps of 128 entries
 constexpr uint32_t kQcMaxFast = 511u;        // largest count that takes the shared-memory path
 static_assert(512 + 3 * kQcWarps * kQcRowsPerGrab + 64 <= 1020, "QC pass: too many rows in flight for the lazy flush");
 
@@ -95,7 +98,12 @@ __device__ __noinline__ void qc_check_table(uint32_t* qsm, int G, int lane, uint
   }
 }
 
-template <bool SPLITS>
+// NB > 0: the table's NB interior entries (need[1 .. NB]; need[0] = 0 and need[NB + 1] = K are
+// the trivial ones) are counted while the row streams by, from the columns the lanes hold anyway:
+// an interior step asks one vote "is my quad's last column below the bound?" (rows are sorted, so
+// the lanes below form a prefix), an edge step counts entry by entry.  NB = 0 with SPLITS: binary
+// searches in the row after it was streamed (any number of entries).
+template <bool SPLITS, int NB>
 __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a) {
   extern __shared__ __align__(16) uint32_t qsm[];      // [G] packed flag | count | total, + 1 spare
   const int G = a.n_cols;
@@ -105,6 +113,7 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
   asm volatile("mov.u32 %0, %0;" : "+r"(sbase));       // keep it in a register
   __shared__ unsigned s_rows;
   __shared__ volatile unsigned s_chk;
+  const uint64_t pol = l2_evict_first_policy();
 
   for (int g = tid; g <= G; g += kQcThreads)
     qsm[g] = (g < G && a.flags != nullptr && a.flags[g] != 0) ? 0x80000000u : 0u;
@@ -134,8 +143,13 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
   auto l2_prefetch = [&](int64_t p0) {
     const int64_t p = p0 + lane * 32;
     if (lane < 4 && p < a.nnz) {
+#if RSC_QC_EVICT & 2
+      asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(a.indices + p));
+      asm volatile("prefetch.global.L2::evict_last [%0];" ::"l"(a.data + p));
+#else
       asm volatile("prefetch.global.L2 [%0];" ::"l"(a.indices + p));
       asm volatile("prefetch.global.L2 [%0];" ::"l"(a.data + p));
+#endif
     }
   };
   auto opaque = [](int v) -> int { asm volatile("mov.u32 %0, %0;" : "+r"(v)); return v; };
@@ -212,13 +226,15 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
       const int64_t nptr = next_ok ? load_ptrs(rnext) : 0;
       const int nr = (int)min((long long)kQcRowsPerGrab, a.n_rows - r0);
       const int64_t gend = __shfl_sync(0xffffffffu, mptr, nr);   // end of the grab's contiguous range
+      // where the look-ahead continues once it runs past gend: the head of the next grab.  The
+      // distance stays kQcAhead steps across the grab boundary -- fetching that head any earlier
+      // (a whole row ahead) lets part of it fall out of L2 again before it is used
+      const int64_t nhead = next_ok ? (__shfl_sync(0xffffffffu, nptr, 0) & ~3LL) : a.nnz;
 #pragma unroll 1
       for (int ri = 0; ri < nr; ++ri) {
         const long long row = r0 + ri;
         const int64_t beg = __shfl_sync(0xffffffffu, mptr, ri);
         const int64_t end = __shfl_sync(0xffffffffu, mptr, ri + 1);
-        if (ri == 1 && next_ok)                         // the head of the next grab
-          for (int i = 0; i < kQcAhead; ++i) l2_prefetch((__shfl_sync(0xffffffffu, nptr, 0) & ~3LL) + i * 128);
         // quads at 16-byte aligned offsets; e = index relative to the row start.  The lane's
         // pointers / e0 advance by 128 entries per step (no per-step address arithmetic).
         const int64_t abeg = beg & ~3LL;
@@ -226,6 +242,9 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
         const int len = (int)(end - beg);
         const int span = opaque(len > 0 ? head + len : 0);
         t32 = 0; m32 = 0; n32 = 0; T64 = 0; M64 = 0;
+        int cnt_i[NB > 0 ? NB : 1], cnt_e[NB > 0 ? NB : 1];   // entries below bound b: interior steps (warp-uniform) / edge steps (per lane)
+#pragma unroll
+        for (int b = 0; b < NB; ++b) { cnt_i[b] = 0; cnt_e[b] = 0; }
         uint32_t* sp = SPLITS ? a.splits + (size_t)row * (size_t)(K + 1) : nullptr;
         const int32_t* ip = a.indices + abeg + lane * 4;
         const float* dp = a.data + abeg + lane * 4;
@@ -235,8 +254,13 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
         auto load_q = [&](const int32_t* ipq, const float* dpq, int e, int4& jv, float4& xv) {
           if (e >= len) return;                         // quad past the row
           if (vec_ok) {
+#if RSC_QC_EVICT & 1
+            jv = ldg_stream_i4(ipq, pol);
+            xv = ldg_stream_f4(dpq, pol);
+#else
             jv = __ldg(reinterpret_cast<const int4*>(ipq));
             xv = __ldg(reinterpret_cast<const float4*>(dpq));
+#endif
           } else {
             jv = make_int4(0, 0, 0, 0);
             xv = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -255,13 +279,42 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
           const int4 jc = jn;
           const float4 xc = xn;
           load_q(ip + 128, dp + 128, e0 + 128, jn, xn);
-          if (pf < gend) l2_prefetch(pf);
+          l2_prefetch(pf < gend ? pf : nhead + ((pf - gend) & ~127LL));
           const bool inter = (base > 0 || head == 0) && (base + 128 <= span);
-          if (inter) quad(std::false_type{}, jc, xc, e0, len);
-          else if (e0 < len) quad(std::true_type{}, jc, xc, e0, len);
+          if (inter) {
+            quad(std::false_type{}, jc, xc, e0, len);
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+              if (cnt_i[b] >= 0) {                      // warp-uniform: the bound was not crossed yet
+                const int32_t bound = a.need[b + 1] << RSC_SPLIT_SHIFT;
+                const unsigned mge = __ballot_sync(0xffffffffu, jc.w >= bound);
+                if (mge == 0u) {
+                  cnt_i[b] += 128;
+                } else {                                // the crossing step: count it, then stop looking
+                  const int L = __ffs(mge) - 1;
+                  const int part = (jc.x < bound ? 1 : 0) + (jc.y < bound ? 1 : 0) + (jc.z < bound ? 1 : 0);
+                  cnt_i[b] = ~(cnt_i[b] + 4 * L + __shfl_sync(0xffffffffu, part, L));
+                }
+              }
+            }
+          } else if (e0 < len) {
+            quad(std::true_type{}, jc, xc, e0, len);
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+              const int32_t bound = a.need[b + 1] << RSC_SPLIT_SHIFT;
+              cnt_e[b] += ((unsigned)(e0 + 0) < (unsigned)len && jc.x < bound ? 1 : 0) +
+                          ((unsigned)(e0 + 1) < (unsigned)len && jc.y < bound ? 1 : 0) +
+                          ((unsigned)(e0 + 2) < (unsigned)len && jc.z < bound ? 1 : 0) +
+                          ((unsigned)(e0 + 3) < (unsigned)len && jc.w < bound ? 1 : 0);
+            }
+          }
           ip += 128; dp += 128; e0 += 128; pf += 128;
         }
-        if (SPLITS) {
+        if (SPLITS && NB > 0) {
+          // cnt_i is stored complemented once the bound was crossed in an interior step.  NB = 1:
+          // the edge-step count rides in the upper half of n32 (both < 2^16: n_cols < 57 841)
+          if (NB == 1) n32 += (unsigned)cnt_e[0] << 16;
+        } else if (SPLITS) {
           // split table of the row: lane k finds #{entries with column < k * RSC_SPLIT_WIDTH} by
           // binary search in the (sorted) row, whose lines were just streamed (L2 / L1 hits)
           // (all K + 1 entries, or only the listed ones: fewer probing lanes, less re-read traffic)
@@ -287,7 +340,21 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
           T = (long long)warp_sum(t32);
           M = (long long)warp_sum(m32);
         }
-        const int N = (int)warp_sum(n32);
+        int N = (int)warp_sum(n32);
+        if (SPLITS && NB > 0) {
+          int lo[NB > 0 ? NB : 1];
+#pragma unroll
+          for (int b = 0; b < NB; ++b) {
+            const int ci = cnt_i[b] < 0 ? ~cnt_i[b] : cnt_i[b];
+            lo[b] = ci + (NB == 1 ? (N >> 16) : warp_sum(cnt_e[b]));
+          }
+          if (NB == 1) N &= 0xffff;
+          // lanes 0 .. NB + 1 write one entry each
+          uint32_t v = lane == 0 ? 0u : (uint32_t)len;
+#pragma unroll
+          for (int b = 0; b < NB; ++b) if (lane == b + 1) v = (uint32_t)lo[b];
+          if (lane <= NB + 1) sp[a.need[lane]] = v;
+        }
         if (lane == 0) {
           if (a.cell_total) a.cell_total[row] = T;
           if (a.cell_total_f32) a.cell_total_f32[row] = (float)T;
@@ -392,24 +459,28 @@ int launch_qc(const rsc_csr& X, const uint8_t* gene_flags, int64_t* cell_total_i
     for (int i = 0; i < n_need_blocks; ++i) a.need[i] = need_blocks[i];
   }
   a.row_counter = static_cast<unsigned long long*>(ws);
-  static bool attr_set = false;
-  if (!attr_set) {
-    RSC_CUDA(cudaFuncSetAttribute(qc_stream_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)kMaxDynSmem));
-    RSC_CUDA(cudaFuncSetAttribute(qc_stream_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)kMaxDynSmem));
-    attr_set = true;
-  }
   a.check_shift = 0u;                                           // largest power of two <= the option (<= 512)
   while (a.check_shift < 9u && (2u << a.check_shift) <= (uint32_t)g_opt.qc_row_budget) ++a.check_shift;
   a.flush_all = g_opt.flush_all ? 1u : 0u;
   int64_t blocks = (X.n_rows + kQcWarps * kQcRowsPerGrab - 1) / (kQcWarps * kQcRowsPerGrab);
   const int cap = g_opt.grid_ctas > 0 ? g_opt.grid_ctas : sm_count();
   if (blocks > cap) blocks = cap;
-  if (row_splits != nullptr)
-    qc_stream_kernel<true><<<(unsigned)blocks, kQcThreads, smem, st>>>(a);
-  else
-    qc_stream_kernel<false><<<(unsigned)blocks, kQcThreads, smem, st>>>(a);
+  // in-stream counting serves a list {0, k1 < .. < kNB, K} with 1 <= NB <= 3 interior entries
+  int nb = 0;
+  if (row_splits != nullptr && a.n_need >= 3 && a.n_need <= 5 && a.need[0] == 0 &&
+      a.need[a.n_need - 1] == a.n_fine) {
+    nb = a.n_need - 2;
+    for (int i = 1; i < a.n_need; ++i)
+      if (a.need[i] <= a.need[i - 1]) nb = 0;
+  }
+  void (*kern)(const QcArgs) = qc_stream_kernel<false, 0>;
+  if (row_splits != nullptr) {
+    kern = nb == 1 ? qc_stream_kernel<true, 1> : nb == 2 ? qc_stream_kernel<true, 2>
+         : nb == 3 ? qc_stream_kernel<true, 3> : qc_stream_kernel<true, 0>;
+  }
+  // the attribute is per device: set on every launch (cheap), not cached per process
+  RSC_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem));
+  kern<<<(unsigned)blocks, kQcThreads, smem, st>>>(a);
   RSC_LAUNCH_CHECK("qc_stream_kernel");
   return RSC_OK;
 }
