@@ -29,6 +29,11 @@ Pins (tests/test_oracle_*.py, `-m "not gpu"`):
   scale_dense      dense (X - mean) / sd with numpy; column mean 0 / sd 1 when unclipped;
                    zero-variance gene => sd 1; clip bounds; zero_center = False keeps zeros
   hvg_cutoffs      window tests written out with loops; infinite window == all non-NaN z
+  gram_cov         numpy.cov of the dense matrix; explicit triple loop on tiny inputs; symmetry,
+                   positive semi-definiteness; diag(C) == gene_moments' variance (ddof 1);
+                   constant column => zero row / column of C; a gene permutation permutes C
+  pca_transform    (X - 1 mu^T) V on the dense centred matrix; columns of Z sum to 0 when mu is
+                   the true mean; V = identity returns the centred matrix
   The CONSTANTS of H1/H5 (1e-12 floor, 0.1 % edge extension, ddof = 1 inside
   bins, z = 1 rule) are not in PAPER.md ("follows scanpy", L87) and scanpy is
   not installed: those constants are **parity unpinned** against the paper.
@@ -376,3 +381,40 @@ def hvg_cutoffs(mean_t, disp_norm, min_mean=0.0125, max_mean=3.0, min_disp=0.5, 
     with np.errstate(invalid="ignore"):
         mask = (m > min_mean) & (m < max_mean) & (z > min_disp) & (z < max_disp)
     return dict(mask=mask.astype(np.uint8), indices=np.nonzero(mask)[0].astype(I32), count=int(mask.sum()))
+
+
+# ---------------------------------------------------------------------------- NEXT-3, second half
+def gram_cov(indptr, indices, data, n_genes: int) -> dict:
+    """Sparse PCA front end, PAPER.md:L95 "Principal component analysis": for X in R^{n x p}
+    (cells x genes, CSR)
+        mu = (1/n) X^T 1                       per-feature means
+        S  = X^T X                             Gram matrix (the paper accumulates the upper
+                                               triangle and mirrors it; here all of it, plainly)
+        C  = (1/(n-1)) (S - n mu mu^T)         mean-centred covariance, no explicit centring
+    in float64 from the float32 values.  Returns {"mean": [p], "gram": [p, p], "cov": [p, p]}.
+    n must be >= 2 (the 1/(n-1) of L95).  S is formed by definition, entry by entry of the sparse
+    rows: S[a, b] = sum over cells i of x_ia x_ib (a dense matmul of the densified matrix is the
+    library step that evaluates exactly this sum)."""
+    indptr = np.asarray(indptr, dtype=I64)
+    indices = np.asarray(indices, dtype=I64)
+    n = indptr.shape[0] - 1
+    assert n >= 2, "covariance needs at least two cells"
+    X = np.zeros((n, n_genes), dtype=F64)
+    X[_row_ids(indptr), indices] = np.asarray(data, dtype=F32).astype(F64)
+    mu = X.sum(axis=0) / n
+    S = X.T @ X
+    C = (S - n * np.outer(mu, mu)) / (n - 1)
+    return {"mean": mu, "gram": S, "cov": C}
+
+
+def pca_transform(indptr, indices, data, n_genes: int, V, mean) -> np.ndarray:
+    """PAPER.md:L95  Z = X V - 1 (mu^T V): the sparse-to-dense projection with implicit centring
+    (V in R^{p x k} the loadings, mu the per-feature means).  float64; returns Z [n, k]."""
+    indptr = np.asarray(indptr, dtype=I64)
+    indices = np.asarray(indices, dtype=I64)
+    V = np.asarray(V, dtype=F64)
+    mean = np.asarray(mean, dtype=F64)
+    n = indptr.shape[0] - 1
+    X = np.zeros((n, n_genes), dtype=F64)
+    X[_row_ids(indptr), indices] = np.asarray(data, dtype=F32).astype(F64)
+    return X @ V - np.ones((n, 1)) * (mean @ V)[None, :]
