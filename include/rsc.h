@@ -274,6 +274,26 @@ int rsc_scale_dense(const rsc_csr* X, const double* gene_mean, const double* gen
                     void* stream);
 
 /* ---------------------------------------------------------------------------------
+ * SURVEY.md 8(f) NEXT-3 (second half) -- rsc_gram_cov: the sparse PCA front end of PAPER.md:L95
+ * ("Principal component analysis"; L137 "centered Gram matrix construction") for X in R^{n x p}
+ * (run it on the HVG-subset, log-normalised matrix):
+ *     out_mean[j]    mu = (1/n) X^T 1                                  double[p]
+ *     out_gram[a][b] S  = X^T X (upper triangle accumulated, mirrored) double[p * p], row-major
+ *     out_cov[a][b]  C  = (S - n mu mu^T) / (n - 1)  (implicit centring) double[p * p]
+ *   Any output may be NULL.  The contraction runs on the tensor cores (tcgen05, fp32 accumulators
+ *   in TMEM) on fp16 pairs hi + lo of x * 2^k (2^k chosen on the device from max |x|; 22
+ *   significand bits), S = hi^T hi + hi^T lo + lo^T hi: fp32-equivalent accuracy, |S - S_exact| <=
+ *   1e-5 |S_exact| entry-wise for non-negative data (DESIGN.md section 6 gives the budget); C is
+ *   formed from S and the exact mu in double, so its error is that of S divided by n - 1.
+ *   The result is bit-reproducible (no atomics).  n_rows >= 2, 1 <= n_cols <= 8192, |x| finite;
+ *   rows need not be sorted.  ws: rsc_gram_cov_workspace_bytes(n_rows, n_cols, nnz) bytes (two
+ *   dense fp16 planes of at most 262 144 rows, the partial tiles; <= 2 x 4.3 GB + 0.6 GB).
+ * ------------------------------------------------------------------------------- */
+size_t rsc_gram_cov_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
+int rsc_gram_cov(const rsc_csr* X, double* out_mean, double* out_gram, double* out_cov,
+                 void* ws, size_t ws_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------
  * rsc_hvg_select — Seurat-flavour highly-variable-gene selection on the device
  * ("based on per-gene mean and variance"; L39 "gene selection" kernel
  * that avoids CPU<->GPU transfers; L87 "follow the algorithmic implementations of

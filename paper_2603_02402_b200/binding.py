@@ -41,6 +41,7 @@ EXPORTS = [
     "rsc_hvg_select_workspace_bytes", "rsc_hvg_select",
     "rsc_filter_masks", "rsc_subset_csr_workspace_bytes", "rsc_subset_csr_plan", "rsc_subset_csr_fill",
     "rsc_scale_dense_workspace_bytes", "rsc_scale_dense", "rsc_hvg_cutoffs",
+    "rsc_gram_cov_workspace_bytes", "rsc_gram_cov",
     "rsc_preprocess_workspace_bytes", "rsc_preprocess",
     "rsc_preprocess_host_workspace_bytes", "rsc_preprocess_host",
 ]
@@ -108,6 +109,8 @@ def lib() -> C.CDLL:
     L.rsc_hvg_select_workspace_bytes.argtypes = [i32, i32]
     L.rsc_subset_csr_workspace_bytes.argtypes = [i64, i32]
     L.rsc_scale_dense_workspace_bytes.argtypes = [i32]
+    L.rsc_gram_cov_workspace_bytes.argtypes = [i64, i32, i64]
+    L.rsc_gram_cov.argtypes = [p, p, p, p, p, sz, p]
     L.rsc_hvg_cutoffs.argtypes = [i32, p, p, C.c_double, C.c_double, C.c_double, C.c_double, p, p, p, p]
     L.rsc_scale_dense.argtypes = [p, p, p, flt, C.c_int, p, p, sz, p]
     L.rsc_filter_masks.argtypes = [i64, i32, p, p, p, p, p, p, p, p, p]
@@ -532,6 +535,22 @@ def rsc_scale_dense(X: Csr, gene_mean: torch.Tensor, gene_var: torch.Tensor,
 
 
 # --------------------------------------------------------------------------- NEXT-4 (part): cutoffs
+def rsc_gram_cov(X: Csr, want_gram: bool = True, want_cov: bool = True, stream=None) -> dict:
+    """PAPER.md:L95 mu, S = X^T X, C = (S - n mu mu^T) / (n - 1) on the tensor cores (float64 outputs)."""
+    _need_cuda(X)
+    L, dev, G = lib(), X.device, X.n_cols
+    out = {"mean": torch.empty(G, dtype=torch.float64, device=dev)}
+    if want_gram:
+        out["gram"] = torch.empty(G, G, dtype=torch.float64, device=dev)
+    if want_cov:
+        out["cov"] = torch.empty(G, G, dtype=torch.float64, device=dev)
+    ws = _ws(L.rsc_gram_cov_workspace_bytes(X.n_rows, G, X.nnz), dev)
+    cs = X.c_struct()
+    _check(L.rsc_gram_cov(C.byref(cs), _ptr(out["mean"]), _ptr(out.get("gram")), _ptr(out.get("cov")),
+                          _ptr(ws), ws.numel(), _stream(stream)))
+    return out
+
+
 def rsc_hvg_cutoffs(mean_t: torch.Tensor, disp_norm: torch.Tensor, min_mean: float = 0.0125,
                     max_mean: float = 3.0, min_disp: float = 0.5, max_disp: float = float("inf"),
                     stream=None) -> dict:

@@ -317,6 +317,21 @@ int rsc_hvg_cutoffs(int32_t n_genes, const double* mean_t, const double* disp_no
                             out_indices, out_count, static_cast<cudaStream_t>(stream));
 }
 
+size_t rsc_gram_cov_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz) {
+  return gram_workspace_bytes(n_rows, n_cols, nnz);
+}
+
+int rsc_gram_cov(const rsc_csr* X, double* out_mean, double* out_gram, double* out_cov, void* ws,
+                 size_t ws_bytes, void* stream) {
+  int rc = check_csr(X, "rsc_gram_cov", true);
+  if (rc) return rc;
+  RSC_CHECK_ARG(X->n_rows >= 2, "rsc_gram_cov: needs at least two cells");
+  RSC_CHECK_ARG(gram_supported(X->n_cols), "rsc_gram_cov: n_cols must be in [1, 8192]");
+  if ((rc = check_device())) return rc;
+  if ((rc = check_ws("rsc_gram_cov", ws, ws_bytes, gram_workspace_bytes(X->n_rows, X->n_cols, X->nnz)))) return rc;
+  return launch_gram_cov(*X, out_mean, out_gram, out_cov, ws, ws_bytes, static_cast<cudaStream_t>(stream));
+}
+
 size_t rsc_scale_dense_workspace_bytes(int32_t n_cols) { return scale_workspace_bytes(n_cols); }
 
 int rsc_scale_dense(const rsc_csr* X, const double* gene_mean, const double* gene_var,

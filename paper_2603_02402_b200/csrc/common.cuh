@@ -118,6 +118,11 @@ size_t scale_workspace_bytes(int32_t n_cols);
 int launch_scale_dense(const rsc_csr& X, const double* gene_mean, const double* gene_var,
                        float max_value, int zero_center, float* out, void* ws, cudaStream_t st);
 
+size_t gram_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
+bool gram_supported(int32_t n_cols);
+int launch_gram_cov(const rsc_csr& X, double* out_mean, double* out_gram, double* out_cov, void* ws,
+                    size_t ws_bytes, cudaStream_t st);
+
 // ---- device helpers ----------------------------------------------------------------
 #ifdef __CUDACC__
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }

@@ -1,0 +1,71 @@
+"""GPU parity of rsc_gram_cov (second half) against
+oracle_np.gram_cov: mean at 1e-12, Gram matrix entry-wise at 1e-5 relative (the paper's own
+allclose bar, L155; DESIGN.md section 6 gives the error budget of the fp16-pair tensor-core
+contraction), covariance within the same absolute error divided by n - 1."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle_np as O
+from paper_2603_02402_b200 import Csr, binding as B, synth
+
+pytestmark = pytest.mark.gpu
+
+GRAM_RTOL = 1e-5
+
+
+def _log_csr(n, G, seed, depth, sort=True):
+    indptr, indices, data, _ = synth.small_nb_csr(n, G, seed, depth)
+    dl = np.log1p(data.astype(np.float64)).astype(np.float32)
+    if not sort:                                         # reverse every row: unsorted columns
+        for i in range(n):
+            s, e = indptr[i], indptr[i + 1]
+            indices[s:e] = indices[s:e][::-1].copy()
+            dl[s:e] = dl[s:e][::-1].copy()
+    return indptr, indices, dl
+
+
+def _check(ip, ix, dl, G, sorted_rows=True):
+    X = Csr(torch.from_numpy(ip).cuda(), torch.from_numpy(ix).cuda(), torch.from_numpy(dl).cuda(), G,
+            sorted_indices=sorted_rows)
+    out = B.rsc_gram_cov(X)
+    torch.cuda.synchronize()
+    ref = O.gram_cov(ip, ix, dl, G)
+    n = len(ip) - 1
+    mean, S, Cv = out["mean"].cpu().numpy(), out["gram"].cpu().numpy(), out["cov"].cpu().numpy()
+    np.testing.assert_allclose(mean, ref["mean"], rtol=1e-12, atol=0)
+    assert np.array_equal(S, S.T) and np.array_equal(Cv, Cv.T)          # mirrored, bit for bit
+    err = np.abs(S - ref["gram"])
+    assert np.all(err <= GRAM_RTOL * np.abs(ref["gram"])), (err.max(), (err / np.maximum(np.abs(ref["gram"]), 1e-300)).max())
+    assert np.all((ref["gram"] == 0) <= (S == 0))                       # structural zeros stay exact zeros
+    cerr = np.abs(Cv - ref["cov"])
+    bound = GRAM_RTOL * np.abs(ref["gram"]) / (n - 1) + 1e-12 * np.abs(ref["cov"]) + 1e-300
+    assert np.all(cerr <= bound + 4e-16 * n * np.abs(np.outer(ref["mean"], ref["mean"])) / (n - 1))
+    return out
+
+
+@pytest.mark.parametrize("n,G,seed,depth", [(300, 100, 0, 1.0), (1000, 300, 1, 0.6), (4097, 700, 2, 0.4),
+                                             (2500, 64, 3, 2.0), (33, 129, 4, 1.0)])
+def test_gram_cov_small(n, G, seed, depth):
+    ip, ix, dl = _log_csr(n, G, seed, depth)
+    _check(ip, ix, dl, G)
+
+
+def test_gram_cov_unsorted_rows_and_reproducible():
+    ip, ix, dl = _log_csr(700, 260, 5, 0.8, sort=False)
+    a = _check(ip, ix, dl, 260, sorted_rows=False)
+    b = _check(ip, ix, dl, 260, sorted_rows=False)
+    assert torch.equal(a["gram"], b["gram"]) and torch.equal(a["cov"], b["cov"])   # no atomics: same bits
+
+
+def test_gram_cov_hvg_subset_of_cfg1():
+    """raw counts -> chain -> HVG subset -> Gram / covariance, the workflow order of L47."""
+    cfg = synth.scaled(synth.CONFIGS[1], 3000)
+    indptr, indices, data = synth.make_csr(cfg, "cuda")
+    flags = synth.gene_flags(cfg, "cuda")
+    X = Csr(indptr, indices, data, cfg.n_genes)
+    out = B.rsc_preprocess(X, flags, cfg.target_sum, 1500, cfg.n_bins)
+    Y, g2 = B.rsc_subset_csr(X, None, out["hvg_mask"])
+    torch.cuda.synchronize()
+    ip, ix, dl = Y.indptr.cpu().numpy(), Y.indices.cpu().numpy(), Y.data.cpu().numpy()
+    _check(ip, ix, dl, g2)
