@@ -58,6 +58,10 @@ constexpr int kFuThreads = RSC_FU_THREADS;
 #define RSC_FU_RG 2
 #endif
 constexpr int kFuRowsPerGrab = RSC_FU_RG;
+#ifndef RSC_FU_HEAD
+#define RSC_FU_HEAD 1024
+#endif
+constexpr int kFuHead = RSC_FU_HEAD;              // entries of a segment requested from L2 before the segment is walked
 constexpr long long kCheckBit = 1LL << 62;  // set in a grab's result: this grab crossed a check point
 constexpr int kMaxGroups = 64;
 // rows a CTA can add between two checks of a gene: the check interval (<= 512) + the grabs its
@@ -818,12 +822,26 @@ __device__ __forceinline__ void fused_stream_body(const FusedArgs& a, uint32_t* 
         if (!MOM) ms = cell_scale(a.target_sum, a.cell_total[row]);
       }
     };
-    auto l2_prefetch = [&](int64_t mb, int64_t me, int ri) {   // the 128-byte lines of one segment
+    // L2 look-ahead.  The head of the NEXT segment (its first kFuHead entries: one 128-byte line
+    // per lane and array) is requested when the current segment starts; a segment longer than
+    // that requests its own later parts kFuHead entries ahead while it is walked (lookahead_in).
+    // The distance is bounded on purpose: fetching a whole long segment early (config 5: rows of
+    // up to 25 000 entries) pushes lines out of the L2 before they are used.
+    auto l2_prefetch = [&](int64_t mb, int64_t me, int ri) {
       const int64_t pb = __shfl_sync(0xffffffffu, mb, ri);
       const int64_t pe = __shfl_sync(0xffffffffu, me, ri);
-      for (int64_t p = (pb & ~31LL) + lane * 32; p < pe; p += 32 * 32) {
+      const int64_t pcap = (int64_t)(pb & ~31LL) + kFuHead;
+      const int64_t pe2 = pe < pcap ? pe : pcap;
+      for (int64_t p = (pb & ~31LL) + lane * 32; p < pe2; p += 32 * 32) {
         asm volatile("prefetch.global.L2 [%0];" ::"l"(a.indices + p));
         asm volatile("prefetch.global.L2 [%0];" ::"l"(a.data + p));
+      }
+    };
+    auto lookahead_in = [&](int64_t abeg, int span, int st) {  // st % 4 == 0: entries [st 128 + kFuHead, + 512) of this segment
+      const int off = st * 128 + kFuHead + lane * 32;
+      if (lane < 16 && off < span) {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(a.indices + abeg + off));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(a.data + abeg + off));
       }
     };
     long long r0 = __shfl_sync(0xffffffffu, grab_issue(), 0) & ~kCheckBit;
@@ -914,6 +932,7 @@ __device__ __forceinline__ void fused_stream_body(const FusedArgs& a, uint32_t* 
           for (int st = 0; st < nsteps; ++st) {
             const int4 jc = jn;
             const float4 xc = xn4;
+            if ((st & 3) == 0 && st * 128 + kFuHead < S.head + S.len) lookahead_in(S.abeg, S.head + S.len, st);
             if (st + 1 < nsteps) {
               load_step(S, st + 1, jn, xn4);
             } else {                                      // prefetch the next segment's first step

@@ -1,16 +1,18 @@
 """Row-sharded multi-GPU chain: one process per GPU, each holding a shard of the cells.
 
-The paper scales out by partitioning the matrix "into chunks along the cell axis"
-(Dask).  Here the same partitioning runs as one process per GPU over
-`torch.distributed`: per-cell outputs, normalisation and log1p are independent per row; the
-per-gene integer counts / totals and the double-precision sums S1, S2 need exactly ONE
-exchange each — an all-reduce(sum) of a contiguous per-gene block (<= 36 k genes x 4
-doubles ~ 1.2 MB, latency-bound on NVLink) — after which every rank finalises the moments
-with the global cell count and runs the identical HVG selection.
+The paper scales out by partitioning the matrix "into chunks along the cell axis ... distributed
+evenly across available devices" (Dask).  Here the same partitioning runs as one
+process per GPU over `torch.distributed`: per-cell outputs, normalisation and log1p are
+independent per row; the per-gene integer counts / totals and the double-precision sums S1, S2
+need ONE exchange -- an all-reduce(sum) of one contiguous per-gene block (<= 36 k genes x 6 values
+~ 1.7 MB, latency-bound on NVLink) AFTER the fused pass (the fused pass balances its gene groups
+with the LOCAL counts, which serve as well as the global ones; nothing waits on a collective
+between the two streaming passes) -- after which every rank finalises the moments with the global
+cell count and runs the identical HVG selection.  Shards are cut by stored entries, not by rows
+(`nnz_balanced_rows`; BASELINE.json config 5's row lengths span 50 .. 25 000).
 
-`allreduce_gene_stats` is device-agnostic (it only packs, all-reduces and unpacks), so the
-host-side logic is covered by world_size-2 gloo tests on CPU; the kernels are the same
-single-GPU C-ABI calls.
+`allreduce_gene_stats`, `nnz_balanced_rows` and `shard_csr` are device-agnostic, so the host-side
+logic is covered by world_size-2 gloo tests on CPU; the kernels are the same single-GPU C-ABI calls.
 """
 from __future__ import annotations
 
@@ -23,11 +25,46 @@ import torch.distributed as dist
 from . import binding as B
 
 
+def nnz_balanced_rows(indptr: torch.Tensor, world: int):
+    """Cut the rows into `world` contiguous shards holding (nearly) equal numbers of stored
+    entries: shard k = rows [r_k, r_{k+1}) with r_k = the first row whose offset reaches
+    k * nnz / world.  Returns [(r0, r1)] * world (empty shards possible when world > rows)."""
+    ip = torch.as_tensor(indptr)
+    n = ip.numel() - 1
+    nnz = int(ip[-1])
+    targets = torch.tensor([(nnz * k) // world for k in range(1, world)], dtype=ip.dtype, device=ip.device)
+    cuts = torch.searchsorted(ip[:-1].contiguous(), targets, right=False).tolist() if world > 1 else []
+    bounds = [0] + [min(max(int(c), 0), n) for c in cuts] + [n]
+    for k in range(1, len(bounds)):
+        bounds[k] = max(bounds[k], bounds[k - 1])
+    return [(bounds[k], bounds[k + 1]) for k in range(world)]
+
+
+def shard_csr(indptr: torch.Tensor, indices: torch.Tensor, data: torch.Tensor, r0: int, r1: int):
+    """Rows [r0, r1) as a CSR of their own (offsets rebased; indices / data are views)."""
+    p0, p1 = int(indptr[r0]), int(indptr[r1])
+    return (indptr[r0:r1 + 1] - p0).contiguous(), indices[p0:p1], data[p0:p1]
+
+
 def allreduce_gene_stats(int_stats: Dict[str, torch.Tensor], f64_stats: Dict[str, torch.Tensor],
-                         group=None) -> None:
-    """In-place all-reduce(sum) of per-gene statistics: all integer arrays travel as one
-    int64 buffer, all float64 arrays as one float64 buffer (two collectives in total)."""
+                         group=None, exact_in_f64: bool = False) -> None:
+    """In-place all-reduce(sum) of per-gene statistics.  All integer arrays travel as one int64
+    buffer and all float64 arrays as one float64 buffer (two collectives, back to back); with
+    exact_in_f64 (the caller guarantees every integer total stays below 2^53) the integers ride
+    in the float64 buffer and ONE collective moves everything."""
     if not dist.is_initialized() or dist.get_world_size(group) == 1:
+        return
+    if exact_in_f64 and int_stats and f64_stats:
+        ki, kf = sorted(int_stats), sorted(f64_stats)
+        flat = torch.cat([int_stats[k].reshape(-1).to(torch.float64) for k in ki] +
+                         [f64_stats[k].reshape(-1) for k in kf])
+        dist.all_reduce(flat, op=dist.ReduceOp.SUM, group=group)
+        off = 0
+        for stats, keys in ((int_stats, ki), (f64_stats, kf)):
+            for k in keys:
+                n = stats[k].numel()
+                stats[k].copy_(flat[off:off + n].reshape(stats[k].shape).to(stats[k].dtype))
+                off += n
         return
     for stats, dt in ((int_stats, torch.int64), (f64_stats, torch.float64)):
         if not stats:
@@ -58,7 +95,7 @@ def _need_blocks(n_cols: int, which_moments: int):
 
 def preprocess_sharded(pp: "B.Preprocessor", X: "B.Csr", gene_flags: Optional[torch.Tensor],
                        events=None, group=None) -> dict:
-    """QC -> all-reduce -> fused pass (raw sums) -> all-reduce -> finalize -> HVG.
+    """QC -> fused pass (raw sums) -> ONE all-reduce of the per-gene block -> finalize -> HVG.
     Per-cell outputs describe the local shard; per-gene outputs and the HVG set are global
     and identical on every rank."""
     L, o, p = B.lib(), pp.out, pp.params
@@ -86,7 +123,6 @@ def preprocess_sharded(pp: "B.Preprocessor", X: "B.Csr", gene_flags: Optional[to
                                      B._ptr(o["gene_n_cells"]), B._ptr(o["gene_total_i64"]),
                                      B._ptr(sh["splits"]), C.cast(sh["need"][0], C.c_void_p),
                                      sh["need"][1], B._ptr(sh["w0"]), sh["w0"].numel(), sp))
-    allreduce_gene_stats({"n_cells": o["gene_n_cells"], "total": o["gene_total_i64"]}, {}, group)
     if events:
         events[1].record(st)
     B._check(L.rsc_normalize_log1p_moments(
@@ -94,7 +130,9 @@ def preprocess_sharded(pp: "B.Preprocessor", X: "B.Csr", gene_flags: Optional[to
         B._ptr(sh["splits"]), p.which_moments, p.ddof, B._ptr(o["mean_log"]), B._ptr(o["var_log"]),
         B._ptr(o["mean_lin"]), B._ptr(o["var_lin"]), B._ptr(sh["sums"]), B._ptr(sh["w1"]),
         sh["w1"].numel(), sp))
-    allreduce_gene_stats({}, {"sums": sh["sums"]}, group)
+    # counts < 2^31 and totals < n_total * 2^24 (QC precondition) are exact in float64 below 2^29 cells
+    allreduce_gene_stats({"n_cells": o["gene_n_cells"], "total": o["gene_total_i64"]}, {"sums": sh["sums"]},
+                         group, exact_in_f64=sh["n_total"] < (1 << 29))
     s = sh["sums"]
     if p.which_moments & B.RSC_MOMENTS_LOG:
         B._check(L.rsc_moments_finalize(G, sh["n_total"], p.ddof, B._ptr(s[0]), B._ptr(s[1]),

@@ -86,13 +86,16 @@ def _chunk_counts(mu: torch.Tensor, gen: torch.Generator) -> torch.Tensor:
     return out
 
 
-def make_csr(cfg: Config, device="cpu", n_cells: Optional[int] = None
+def make_csr(cfg: Config, device="cpu", n_cells: Optional[int] = None, first_rows: Optional[int] = None
              ) -> Tuple[torch.Tensor, torch.Tensor, torch.Tensor]:
     """Draw the configuration's matrix on ``device``.
 
     Returns (indptr int64[n+1], indices int32[nnz], data float32[nnz]).
     ``n_cells`` overrides the row count (used for bounded samples of a
     workload; the gene parameters stay those of the full configuration).
+    ``first_rows`` draws only the first rows OF THE n-CELL MATRIX (whole generation chunks, so
+    at least that many rows come back): the same random numbers in the same order, i.e. a true
+    prefix of the full matrix at a fraction of the cost.
     """
     n = cfg.n_cells if n_cells is None else int(n_cells)
     G = cfg.n_genes
@@ -122,7 +125,8 @@ def make_csr(cfg: Config, device="cpu", n_cells: Optional[int] = None
     row_nnz = torch.empty(n, dtype=torch.int64, device=dev)
 
     pos = 0
-    for r0 in range(0, n, rows_per_chunk):
+    n_draw = n if first_rows is None else min(n, -(-int(first_rows) // rows_per_chunk) * rows_per_chunk)
+    for r0 in range(0, n_draw, rows_per_chunk):
         r1 = min(n, r0 + rows_per_chunk)
         mu = cfg.depth * s[r0:r1, None] * g[None, :]
         if cfg.n_housekeeping:
@@ -139,8 +143,8 @@ def make_csr(cfg: Config, device="cpu", n_cells: Optional[int] = None
         data[pos:pos + k] = x[nz]
         pos += k
         del x, nz, rc
-    indptr = torch.zeros(n + 1, dtype=torch.int64, device=dev)
-    torch.cumsum(row_nnz, dim=0, out=indptr[1:])
+    indptr = torch.zeros(n_draw + 1, dtype=torch.int64, device=dev)
+    torch.cumsum(row_nnz[:n_draw], dim=0, out=indptr[1:])
     return indptr, indices[:pos], data[:pos]
 
 
