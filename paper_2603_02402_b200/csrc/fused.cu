@@ -278,47 +278,67 @@ fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid, f
 // rsc_gene_moments knows nothing about the values, so the plan looks at a sample (32 768 stored
 // entries in 1 024 clusters spread evenly over the matrix): largest value v_max, smallest positive value, and how
 // the entries spread over the column blocks.
-//   * window top 2^E > 2 v_max (one binade of head room over the sample);
-//   * if the sample spans at most kLogBinades - 1 binades below it, the three-word scheme
-//     (12 B / gene), else the five-word scheme (one-word values 2^(E-9) .. 2^E, two-word values
-//     up to 2^(E+10));
+//   * 2^E > v_max of the sample;
+//   * if at most one sampled value in 1024 lies below 2^(E - kLogBinades), the three-word scheme
+//     with the window [2^(E - kLogBinades), 2^E) (12 B / gene), else the five-word scheme (one
+//     binade of head room: one-word values 2^(E-8) .. 2^(E+1), two-word values up to 2^(E+11));
 //   * gene groups as large as the table allows, CTAs dealt by the sampled entry counts.
 // A value the sample did not foresee still lands in the global double sums: correct, only slow.
 __global__ void __launch_bounds__(1024)
 moments_plan_kernel(FusedPlan* plan, int G, int K, int grid, long long n_rows, long long nnz,
                     const int32_t* __restrict__ indices, const float* __restrict__ data) {
   __shared__ double mass[kMaxGroups];
-  __shared__ float s_max[32], s_min[32];
-  __shared__ int s_ng;
+  __shared__ float s_max[32];
+  __shared__ int s_ng, s_E, s_below, s_pos;
   constexpr int kPer = 32;
   const int tid = threadIdx.x;
   // 32 * kPer clusters of 32 consecutive entries (a warp reads one line per load), spread evenly
   const long long step = nnz > 1024LL * kPer ? (nnz - 32) / (32LL * kPer) : 32;
-  float vmax = 0.0f, vmin = INFINITY;
-  int32_t col[kPer];                                      // the sampled entries' columns (registers)
+  float vmax = 0.0f;
+  int32_t col[kPer];                                      // the sampled entries' columns and values (registers)
+  float val[kPer];
 #pragma unroll
   for (int i = 0; i < kPer; ++i) {                        // independent loads: all in flight together
     const long long p = ((long long)i * 32 + (tid >> 5)) * step + (tid & 31);
     float v = 0.0f;
     col[i] = -1;
     if (p < nnz) { v = __ldg(data + p); col[i] = __ldg(indices + p); }
+    val[i] = v;
     if (v > vmax) vmax = v;
-    if (v > 0.0f && v < vmin) vmin = v;
   }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
-    vmin = fminf(vmin, __shfl_xor_sync(0xffffffffu, vmin, o));
-  }
-  if ((tid & 31) == 0) { s_max[tid >> 5] = vmax; s_min[tid >> 5] = vmin; }
+  for (int o = 16; o > 0; o >>= 1) vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
+  if ((tid & 31) == 0) s_max[tid >> 5] = vmax;
   if (tid < kMaxGroups) mass[tid] = 0.0;
+  if (tid == 0) { s_below = 0; s_pos = 0; }
   __syncthreads();
   if (tid == 0) {
-    for (int w = 1; w < 32; ++w) { vmax = fmaxf(vmax, s_max[w]); vmin = fminf(vmin, s_min[w]); }
+    for (int w = 1; w < 32; ++w) vmax = fmaxf(vmax, s_max[w]);
     if (!(vmax > 0.0f) || !isfinite(vmax)) vmax = 1.0f;
     int E;
-    frexp(2.0 * (double)vmax, &E);                         // 2^E > 2 v_max
-    const bool narrow = (double)vmin >= ldexp(1.0, E - kLogBinades);
+    frexp((double)vmax * 1.0000001, &E);                   // 2^E > v_max of the sample
+    s_E = E;
+  }
+  __syncthreads();
+  {
+    // how much of the sample lies below the narrow window [2^(E - kLogBinades), 2^E)?  Up to one
+    // entry in 1024 may (such values take the global double sums: correct, only slower), so a
+    // few deep cells do not force the five-word scheme on everybody else
+    const float bottom = ldexpf(1.0f, s_E - kLogBinades);
+    int below = 0, pos = 0;
+#pragma unroll
+    for (int i = 0; i < kPer; ++i) {
+      pos += val[i] > 0.0f ? 1 : 0;
+      below += (val[i] > 0.0f && val[i] < bottom) ? 1 : 0;
+    }
+    below = warp_sum(below);
+    pos = warp_sum(pos);
+    if ((tid & 31) == 0) { atomicAdd(&s_below, below); atomicAdd(&s_pos, pos); }
+  }
+  __syncthreads();
+  if (tid == 0) {
+    const int E = s_E;
+    const bool narrow = (long long)s_below * 1024 <= (long long)s_pos;
     MomentScale sc;
     sc.pad = 0.0f;
     int bpg;
@@ -328,7 +348,7 @@ moments_plan_kernel(FusedPlan* plan, int G, int K, int grid, long long n_rows, l
       plan->sc_log = sc;
       bpg = kLogWords * 4;
     } else {
-      const int k = 32 - E;
+      const int k = 32 - (E + 1);                          // one binade of head room over the sample
       sc.mult = (float)ldexp(1.0, k); sc.inv1 = ldexp(1.0, -k); sc.inv2 = ldexp(1.0, -2 * k);
       plan->sc_lin = sc;
       bpg = kSetWords * 4;

@@ -11,16 +11,18 @@
 
 namespace rsc {
 
-// per-gene sd (double; 1 where the variance is 0) and the value of a zero entry (float, clipped)
+// per-gene 1 / sd (double; sd = 1 where the variance is 0) and the value of a zero entry (float, clipped)
 __global__ void __launch_bounds__(256)
 scale_prep_kernel(int32_t G, const double* __restrict__ mean, const double* __restrict__ var,
-                  float max_value, int zero_center, double* __restrict__ sd_out, float* __restrict__ base) {
+                  float max_value, int zero_center, double* __restrict__ inv_sd_out, float* __restrict__ base) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= G) return;
   double sd = sqrt(var[j]);
   if (sd == 0.0) sd = 1.0;
-  sd_out[j] = sd;                                          // the entries divide by sd (as the definition)
-  double b = zero_center ? (0.0 - mean[j]) / sd : 0.0;
+  const double inv = 1.0 / sd;
+  inv_sd_out[j] = inv;                                         // the entries multiply by 1 / sd (one rounding more than
+                                                           // the definition's division, in double: far below float32)
+  double b = zero_center ? (0.0 - mean[j]) * inv : 0.0;
   if (max_value > 0.0f) {
     if (b > (double)max_value) b = (double)max_value;
     if (zero_center && b < -(double)max_value) b = -(double)max_value;
@@ -31,7 +33,7 @@ scale_prep_kernel(int32_t G, const double* __restrict__ mean, const double* __re
 __global__ void __launch_bounds__(256)
 scale_dense_kernel(int64_t n_rows, int32_t G, const int64_t* __restrict__ indptr,
                    const int32_t* __restrict__ indices, const float* __restrict__ data,
-                   const double* __restrict__ mean, const double* __restrict__ sd,
+                   const double* __restrict__ mean, const double* __restrict__ inv_sd,
                    const float* __restrict__ base, float max_value, int zero_center,
                    float* __restrict__ out) {
   const int lane = lane_id();
@@ -52,7 +54,7 @@ scale_dense_kernel(int64_t n_rows, int32_t G, const int64_t* __restrict__ indptr
       const int j = __ldg(indices + p);
       double y = (double)__ldg(data + p);
       if (zero_center) y -= mean[j];
-      y = y / sd[j];
+      y = y * inv_sd[j];
       if (max_value > 0.0f) {
         if (y > (double)max_value) y = (double)max_value;
         if (zero_center && y < -(double)max_value) y = -(double)max_value;
@@ -69,7 +71,7 @@ constexpr int kScaleWarps = 4;
 __global__ void __launch_bounds__(kScaleWarps * 32)
 scale_dense_smem_kernel(int64_t n_rows, int32_t G, const int64_t* __restrict__ indptr,
                         const int32_t* __restrict__ indices, const float* __restrict__ data,
-                        const double* __restrict__ mean, const double* __restrict__ sd,
+                        const double* __restrict__ mean, const double* __restrict__ inv_sd,
                         const float* __restrict__ base, float max_value, int zero_center,
                         float* __restrict__ out) {
   extern __shared__ __align__(16) float srow[];
@@ -80,7 +82,7 @@ scale_dense_smem_kernel(int64_t n_rows, int32_t G, const int64_t* __restrict__ i
   auto zscore = [&](int j, float x) -> float {
     double y = (double)x;
     if (zero_center) y -= mean[j];
-    y = y / sd[j];
+    y = y * inv_sd[j];
     if (max_value > 0.0f) {
       if (y > (double)max_value) y = (double)max_value;
       if (zero_center && y < -(double)max_value) y = -(double)max_value;
@@ -133,10 +135,10 @@ int launch_scale_dense(const rsc_csr& X, const double* gene_mean, const double* 
                        float max_value, int zero_center, float* out, void* ws, cudaStream_t st) {
   if (X.n_rows == 0) return RSC_OK;
   unsigned char* w = static_cast<unsigned char*>(ws);
-  double* sd = reinterpret_cast<double*>(w);
+  double* inv_sd = reinterpret_cast<double*>(w);
   float* base = reinterpret_cast<float*>(w + align_up(sizeof(double) * (size_t)X.n_cols, 256));
   scale_prep_kernel<<<(X.n_cols + 255) / 256, 256, 0, st>>>(X.n_cols, gene_mean, gene_var, max_value,
-                                                            zero_center, sd, base);
+                                                            zero_center, inv_sd, base);
   RSC_LAUNCH_CHECK("scale_prep_kernel");
   const size_t smem = sizeof(float) * (size_t)kScaleWarps * (size_t)X.n_cols;
   const bool staged = (X.n_cols & 3) == 0 && smem <= 100 * 1024 &&
@@ -149,7 +151,7 @@ int launch_scale_dense(const rsc_csr& X, const double* gene_mean, const double* 
     const int64_t cap = (int64_t)sm_count() * (per_sm > 16 ? 16 : per_sm);
     if (blocks > cap) blocks = cap;
     scale_dense_smem_kernel<<<(unsigned)blocks, kScaleWarps * 32, smem, st>>>(
-        X.n_rows, X.n_cols, X.indptr, X.indices, X.data, gene_mean, sd, base, max_value, zero_center, out);
+        X.n_rows, X.n_cols, X.indptr, X.indices, X.data, gene_mean, inv_sd, base, max_value, zero_center, out);
     RSC_LAUNCH_CHECK("scale_dense_smem_kernel");
     return RSC_OK;
   }
@@ -157,7 +159,7 @@ int launch_scale_dense(const rsc_csr& X, const double* gene_mean, const double* 
   const int64_t cap = (int64_t)sm_count() * 16;
   if (blocks > cap) blocks = cap;
   scale_dense_kernel<<<(unsigned)blocks, 256, 0, st>>>(X.n_rows, X.n_cols, X.indptr, X.indices, X.data,
-                                                       gene_mean, sd, base, max_value, zero_center, out);
+                                                       gene_mean, inv_sd, base, max_value, zero_center, out);
   RSC_LAUNCH_CHECK("scale_dense_kernel");
   return RSC_OK;
 }
