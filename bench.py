@@ -55,6 +55,7 @@ def parse_args():
                          "2 linear scale (scanpy's Seurat input), 3 both")
     ap.add_argument("--no-variants", action="store_true",
                     help="skip variants / unfused / next / other configs (headline only)")
+    ap.add_argument("--no-configs", action="store_true", help="skip the other BASELINE.json configs")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -534,7 +535,7 @@ def main():
 
     # ---- the other BASELINE.json configs, same chain, same run
     configs = None
-    if extras and args.cells is None:
+    if extras and args.cells is None and not args.no_configs:
         configs = {}
         others = [c for c in (1, 2, 5, 4) if c != cfgno]
         if args.config != "all":

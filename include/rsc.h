@@ -324,6 +324,11 @@ int rsc_hvg_select(int32_t n_genes, const double* gene_mean, const double* gene_
  * rsc_qc_metrics -> rsc_normalize_log1p_moments -> rsc_hvg_select (fed with the
  * linear-scale moments when hvg_on_linear != 0, else the log-scale ones; DESIGN.md
  * reading R8).  `out` collects the device output pointers; see rsc_outputs.
+ * PRECONDITION (as rsc_qc_metrics): X->data holds integer counts.  The chain normalises with the
+ * QC totals, which truncate every value to an integer before summing (reading R4); for
+ * non-integer input (ambient-corrected or already normalised values) the row sums of x' then
+ * differ from target_sum and nothing reports it -- call rsc_normalize_total with a NULL total
+ * (float row sums), rsc_log1p and rsc_gene_moments instead.
  * ------------------------------------------------------------------------------- */
 typedef struct {
   /* per cell [n_rows] */

@@ -32,6 +32,11 @@ Pins (tests/test_oracle_*.py, `-m "not gpu"`):
   gram_cov         numpy.cov of the dense matrix; explicit triple loop on tiny inputs; symmetry,
                    positive semi-definiteness; diag(C) == gene_moments' variance (ddof 1);
                    constant column => zero row / column of C; a gene permutation permutes C
+  hvg_cell_ranger  percentile_linear == numpy.percentile; pandas.cut codes on the same edges;
+                   pandas groupby median / MAD restatement; per-bin median of z == 0 and
+                   median |z| == 0.6745; hand-worked fixture tests/golden/hvg_cell_ranger_tiny.txt
+  hvg_merge_batches pandas sort_values([nbatches, zbar], ascending False, NaN last) restatement; one
+                   batch == that batch's own selection; a gene selected everywhere outranks all
   pca_transform    (X - 1 mu^T) V on the dense centred matrix; columns of Z sum to 0 when mu is
                    the true mean; V = identity returns the centred matrix
   The CONSTANTS of H1/H5 (1e-12 floor, 0.1 % edge extension, ddof = 1 inside
@@ -418,3 +423,117 @@ def pca_transform(indptr, indices, data, n_genes: int, V, mean) -> np.ndarray:
     X = np.zeros((n, n_genes), dtype=F64)
     X[_row_ids(indptr), indices] = np.asarray(data, dtype=F32).astype(F64)
     return X @ V - np.ones((n, 1)) * (mean @ V)[None, :]
+
+
+# ---------------------------------------------------------------------------- NEXT-4: other HVG variants
+MAD_SCALE = 0.6744897501960817          # Phi^-1(3/4): MAD / MAD_SCALE estimates sigma for normal data
+
+
+def percentile_linear(sorted_vals: np.ndarray, q_percent: float) -> float:
+    """Linear-interpolation percentile of an ascending array (the textbook definition numpy's
+    default method evaluates): virtual index vi = (q / 100) (n - 1), lo = floor(vi), t = vi - lo,
+    value = a[lo] + (a[hi] - a[lo]) t for t < 0.5, else a[hi] - (a[hi] - a[lo]) (1 - t)
+    (the second form keeps the result exact at t -> 1), with separate multiply and add."""
+    a = np.asarray(sorted_vals, dtype=F64)
+    n = a.shape[0]
+    vi = (F64(q_percent) / F64(100.0)) * F64(n - 1)
+    lo = int(np.floor(vi))
+    hi = min(lo + 1, n - 1)
+    t = F64(vi - F64(lo))
+    diff = F64(a[hi] - a[lo])
+    if t < 0.5:
+        return float(F64(a[lo] + F64(diff * t)))
+    return float(F64(a[hi] - F64(diff * F64(F64(1.0) - t))))
+
+
+def hvg_cell_ranger(gene_mean, gene_var, n_top: int) -> dict:
+    """Cell-ranger-flavour HVG selection ("Highly variable gene
+    selection is based on per-gene mean and variance", L87 "follow the algorithmic implementations
+    of scanpy"; the paper gives no constants -- DESIGN.md reading R18, parity unpinned against
+    PAPER.md).  Input: mean / variance of the NORMALISED, non-logged matrix x'.
+      C1  mean == 0 -> 1e-12;  d = var / mean               (no log transforms)
+      C2  edges = -inf, P10, P15, .., P100 of the means (linear interpolation), +inf;
+          equal edges are merged (an empty interval holds no gene)
+      C3  bin(m) = the interval (e_k, e_{k+1}] that holds m  (right-closed)
+      C4  per bin: med_b = median of the d in the bin, mad_b = median |d - med_b| / 0.6745
+      C5  z = (d - med_b) / mad_b                            (IEEE: mad_b = 0 gives +-inf or NaN)
+      C6  cutoff = n_top-th largest non-NaN z; mask = z is not NaN and z >= cutoff (as H7)
+    Returns disp, disp_norm, bin (index into the merged edges), edges, mask, cutoff, count."""
+    mean = np.asarray(gene_mean, dtype=F64).copy()
+    var = np.asarray(gene_var, dtype=F64)
+    G = mean.shape[0]
+    mean0 = mean.copy()
+    mean0[mean0 == 0] = 1e-12
+    d = var / mean0
+    srt = np.sort(mean)
+    edges = [-np.inf] + [percentile_linear(srt, q) for q in range(10, 105, 5)] + [np.inf]
+    merged = [edges[0]]
+    for e in edges[1:]:
+        if e != merged[-1]:
+            merged.append(e)
+    edges = np.asarray(merged, dtype=F64)
+    nb = edges.shape[0] - 1
+    bins = np.empty(G, dtype=I32)
+    for j in range(G):
+        k = 0
+        while not (mean[j] <= edges[k + 1]):              # smallest k with m <= e_{k+1}
+            k += 1
+        bins[j] = k
+    med = np.full(nb, np.nan)
+    mad = np.full(nb, np.nan)
+    for b in range(nb):
+        sel = (bins == b) & ~np.isnan(d)
+        if sel.any():
+            med[b] = np.median(d[sel])
+            mad[b] = np.median(np.abs(d[sel] - med[b])) / MAD_SCALE
+    with np.errstate(divide="ignore", invalid="ignore"):
+        z = (d - med[bins]) / mad[bins]
+    valid = ~np.isnan(z)
+    k = min(int(n_top), int(valid.sum()))
+    if k > 0:
+        cutoff = np.sort(z[valid])[::-1][k - 1]
+        mask = valid & (z >= cutoff)
+    else:
+        cutoff = np.nan
+        mask = np.zeros(G, dtype=bool)
+    return {"disp": d, "disp_norm": z, "bin": bins, "edges": edges, "median": med, "mad": mad,
+            "mask": mask, "cutoff": cutoff, "count": int(mask.sum()),
+            "indices": np.nonzero(mask)[0].astype(I32)}
+
+
+def hvg_merge_batches(masks, disp_norm, n_top: int) -> dict:
+    """Per-batch HVG (reading R19, scanpy's batch_key convention, parity
+    unpinned against PAPER.md): the selection runs per batch; then per gene
+      B1  nbatches_j = number of batches that selected gene j
+      B2  zbar_j = mean over the batches of the gene's non-NaN normalised dispersions (NaN if none)
+      B3  genes are ranked by (nbatches, zbar) descending, NaN zbar last within its nbatches level;
+          the n_top-th gene of that order sets the cutoff pair and every gene at or above it is
+          selected (ties at the cutoff select more than n_top, as H7).
+    masks: bool [B, G]; disp_norm: float64 [B, G]."""
+    masks = np.asarray(masks).astype(bool)
+    z = np.asarray(disp_norm, dtype=F64)
+    Bn, G = masks.shape
+    nbat = masks.sum(axis=0).astype(I32)
+    cnt = (~np.isnan(z)).sum(axis=0)
+    zs = np.where(np.isnan(z), 0.0, z).sum(axis=0)        # batch order 0 .. B-1: a fixed summation order
+    zbar = np.where(cnt > 0, zs / np.maximum(cnt, 1), np.nan)
+    k = min(int(n_top), G)
+    # rank: nbatches descending, NaN zbar last within a level, then zbar descending
+    order = sorted(range(G), key=lambda j: (-int(nbat[j]), bool(np.isnan(zbar[j])),
+                                            0.0 if np.isnan(zbar[j]) else -zbar[j]))
+    if k > 0:
+        c = order[k - 1]
+        cn, cz, cnan = int(nbat[c]), zbar[c], bool(np.isnan(zbar[c]))
+        mask = np.zeros(G, dtype=bool)
+        for j in range(G):
+            if nbat[j] > cn:
+                mask[j] = True
+            elif nbat[j] == cn:
+                if cnan:
+                    mask[j] = True                        # the cutoff sits in the NaN tail of its level
+                else:
+                    mask[j] = (not np.isnan(zbar[j])) and zbar[j] >= cz
+    else:
+        mask = np.zeros(G, dtype=bool)
+    return {"nbatches": nbat, "disp_norm_mean": zbar, "mask": mask, "count": int(mask.sum()),
+            "indices": np.nonzero(mask)[0].astype(I32)}

@@ -151,9 +151,14 @@ def _stream(stream=None):
     return C.c_void_p(s.cuda_stream)
 
 
-def _ws(nbytes: int, device) -> torch.Tensor:
-    # torch's caching allocator returns 512-byte aligned blocks
-    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+def _ws(nbytes: int, device, stream=None) -> torch.Tensor:
+    # torch's caching allocator returns 512-byte aligned blocks.  A temporary used by kernels
+    # queued on a stream other than the current one is recorded on that stream, so the allocator
+    # does not hand the block out again before those kernels have run.
+    t = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+    if stream is not None and t.is_cuda:
+        t.record_stream(stream)
+    return t
 
 
 @dataclass
@@ -240,7 +245,7 @@ def rsc_qc_metrics(X: Csr, gene_flags: Optional[torch.Tensor] = None, stream=Non
         gene_total_i64=torch.empty(G, dtype=torch.int64, device=dev),
     )
     nb = L.rsc_qc_metrics_workspace_bytes(n, G, X.nnz)
-    ws = _ws(nb, dev)
+    ws = _ws(nb, dev, stream)
     cs = X.c_struct()
     splits = None
     if with_row_splits and X.sorted_indices:
@@ -280,7 +285,7 @@ def rsc_gene_moments(X: Csr, transform: int = 0, ddof: int = 1, stream=None) -> 
     _need_cuda(X)
     L, dev, G = lib(), X.device, X.n_cols
     out = {k: torch.empty(G, dtype=torch.float64, device=dev) for k in ("mean", "var", "sum", "sumsq")}
-    ws = _ws(L.rsc_gene_moments_workspace_bytes(X.n_rows, G, X.nnz), dev)
+    ws = _ws(L.rsc_gene_moments_workspace_bytes(X.n_rows, G, X.nnz), dev, stream)
     cs = X.c_struct()
     _check(L.rsc_gene_moments(C.byref(cs), transform, ddof, _ptr(out["mean"]), _ptr(out["var"]),
                               _ptr(out["sum"]), _ptr(out["sumsq"]), _ptr(ws), ws.numel(),
@@ -304,7 +309,7 @@ def rsc_normalize_log1p_moments(X: Csr, target_sum: float, cell_total_i64: torch
     if which_moments & RSC_MOMENTS_LIN:
         out["mean_lin"] = torch.empty(G, dtype=torch.float64, device=dev)
         out["var_lin"] = torch.empty(G, dtype=torch.float64, device=dev)
-    ws = _ws(L.rsc_normalize_log1p_moments_workspace_bytes(X.n_rows, G, X.nnz), dev)
+    ws = _ws(L.rsc_normalize_log1p_moments_workspace_bytes(X.n_rows, G, X.nnz), dev, stream)
     cs = X.c_struct()
     _check(L.rsc_normalize_log1p_moments(
         C.byref(cs), float(target_sum), _ptr(cell_total_i64), _ptr(gene_n_cells), _ptr(row_splits),
@@ -341,7 +346,7 @@ def rsc_hvg_select(gene_mean: torch.Tensor, gene_var: torch.Tensor, n_top: int, 
         indices=torch.full((G,), -1, dtype=torch.int32, device=dev),
         count=torch.zeros(1, dtype=torch.int32, device=dev),
     )
-    ws = _ws(L.rsc_hvg_select_workspace_bytes(G, n_bins), dev)
+    ws = _ws(L.rsc_hvg_select_workspace_bytes(G, n_bins), dev, stream)
     _check(L.rsc_hvg_select(G, _ptr(gene_mean), _ptr(gene_var), n_top, n_bins, flags,
                             _ptr(out["mean_t"]), _ptr(out["disp"]), _ptr(out["disp_norm"]),
                             _ptr(out["bin"]), _ptr(out["mask"]), _ptr(out["indices"]),
@@ -505,12 +510,14 @@ def rsc_subset_csr(X: Csr, keep_rows: Optional[torch.Tensor] = None,
     the three output sizes (the only synchronisation), allocation, fill."""
     _need_cuda(X)
     L, dev = lib(), X.device
-    ws = _ws(L.rsc_subset_csr_workspace_bytes(X.n_rows, X.n_cols), dev)
+    ws = _ws(L.rsc_subset_csr_workspace_bytes(X.n_rows, X.n_cols), dev, stream)
     out_indptr = torch.empty(X.n_rows + 1, dtype=torch.int64, device=dev)
     counts = torch.zeros(3, dtype=torch.int64, device=dev)
     cs = X.c_struct()
     _check(L.rsc_subset_csr_plan(C.byref(cs), _ptr(keep_rows), _ptr(keep_cols), _ptr(out_indptr),
                                  _ptr(counts), _ptr(ws), ws.numel(), _stream(stream)))
+    if stream is not None:
+        stream.synchronize()                               # .tolist() only waits for the CURRENT stream
     n_out, g_out, nnz_out = (int(v) for v in counts.tolist())
     out_indices = torch.empty(nnz_out, dtype=torch.int32, device=dev)
     out_data = torch.empty(nnz_out, dtype=torch.float32, device=dev)
@@ -526,7 +533,7 @@ def rsc_scale_dense(X: Csr, gene_mean: torch.Tensor, gene_var: torch.Tensor,
     _need_cuda(X)
     L = lib()
     out = torch.empty((X.n_rows, X.n_cols), dtype=torch.float32, device=X.device)
-    ws = _ws(L.rsc_scale_dense_workspace_bytes(X.n_cols), X.device)
+    ws = _ws(L.rsc_scale_dense_workspace_bytes(X.n_cols), X.device, stream)
     cs = X.c_struct()
     _check(L.rsc_scale_dense(C.byref(cs), _ptr(gene_mean), _ptr(gene_var),
                              float(max_value) if max_value is not None else 0.0, int(bool(zero_center)),
@@ -544,7 +551,7 @@ def rsc_gram_cov(X: Csr, want_gram: bool = True, want_cov: bool = True, stream=N
         out["gram"] = torch.empty(G, G, dtype=torch.float64, device=dev)
     if want_cov:
         out["cov"] = torch.empty(G, G, dtype=torch.float64, device=dev)
-    ws = _ws(L.rsc_gram_cov_workspace_bytes(X.n_rows, G, X.nnz), dev)
+    ws = _ws(L.rsc_gram_cov_workspace_bytes(X.n_rows, G, X.nnz), dev, stream)
     cs = X.c_struct()
     _check(L.rsc_gram_cov(C.byref(cs), _ptr(out["mean"]), _ptr(out.get("gram")), _ptr(out.get("cov")),
                           _ptr(ws), ws.numel(), _stream(stream)))

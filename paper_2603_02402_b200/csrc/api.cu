@@ -10,7 +10,7 @@
 namespace rsc {
 
 static thread_local char g_err[512] = "";
-unsigned long long g_launch_count = 0;
+std::atomic<unsigned long long> g_launch_count{0};
 Options g_opt;
 
 void set_error(const char* fmt, ...) {
@@ -20,8 +20,9 @@ void set_error(const char* fmt, ...) {
   va_end(ap);
 }
 
-static int g_dev_checked = -1;   // device ordinal whose capability was verified
-static int g_sm_count = kNumSMs;
+// per host thread (the current device is a per-thread notion): no shared mutable state
+static thread_local int g_dev_checked = -1;   // device ordinal whose capability was verified
+static thread_local int g_sm_count = kNumSMs;
 
 int check_device() {
   int dev = -1;
@@ -100,7 +101,7 @@ extern "C" {
 
 const char* rsc_last_error(void) { return g_err; }
 const char* rsc_version(void) { return "0.1.0"; }
-uint64_t rsc_kernel_launch_count(void) { return g_launch_count; }
+uint64_t rsc_kernel_launch_count(void) { return g_launch_count.load(std::memory_order_relaxed); }
 
 int rsc_set_option(const char* key, long long value) {
   RSC_CHECK_ARG(key != nullptr, "rsc_set_option: key is NULL");

@@ -4,6 +4,8 @@
 
 #include <cuda_runtime.h>
 #include <stdint.h>
+
+#include <atomic>
 #include <stdio.h>
 
 #include "rsc.h"
@@ -38,20 +40,20 @@ void set_error(const char* fmt, ...);
   } while (0)
 
 // run-time tunables (rsc_set_option): defaults are the shipped configuration
-struct Options {
-  int fused_row_budget = 256;     // rows a fused-pass CTA takes between two checks of its tables (<= 256)
-  int flush_all = 0;              // 1: every check moves every gene to the global totals (testing)
-  int qc_row_budget = 512;        // rows a QC CTA takes between two checks of its table (<= 512)
-  int grid_ctas = 0;              // CTAs of the streaming kernels; 0 = one per SM
-  int force_generic = 0;          // 1: always use the generic L2-atomic kernels
+struct Options {                  // process-wide, set through rsc_set_option; atomics: any host thread may set / read
+  std::atomic<int> fused_row_budget{256};     // rows a fused-pass CTA takes between two checks of its tables (<= 256)
+  std::atomic<int> flush_all{0};              // 1: every check moves every gene to the global totals (testing)
+  std::atomic<int> qc_row_budget{512};        // rows a QC CTA takes between two checks of its table (<= 512)
+  std::atomic<int> grid_ctas{0};              // CTAs of the streaming kernels; 0 = one per SM
+  std::atomic<int> force_generic{0};          // 1: always use the generic L2-atomic kernels
 };
 extern Options g_opt;
 
-extern unsigned long long g_launch_count;   // kernels launched by this library (host counter)
+extern std::atomic<unsigned long long> g_launch_count;   // kernels launched by this library (host counter)
 
 #define RSC_LAUNCH_CHECK(name)                                                      \
   do {                                                                              \
-    ++::rsc::g_launch_count;                                                        \
+    ::rsc::g_launch_count.fetch_add(1, std::memory_order_relaxed);                                                      \
     cudaError_t e__ = cudaGetLastError();                                           \
     if (e__ != cudaSuccess) {                                                       \
       ::rsc::set_error("launch of %s failed: %s", name, cudaGetErrorString(e__));   \

@@ -1104,7 +1104,7 @@ fused_finish_kernel(int G, double n, double denom, const FusedPlan* __restrict__
 int launch_fused_generic(const rsc_csr&, float, const int64_t*, int, double*, double*, double*,
                          double*, cudaStream_t);
 
-static int fused_grid() { return g_opt.grid_ctas > 0 ? g_opt.grid_ctas : sm_count(); }
+static int fused_grid() { return g_opt.grid_ctas.load() > 0 ? g_opt.grid_ctas.load() : sm_count(); }
 
 // bytes of shared-memory accumulators per gene
 static int bytes_per_gene(int which) {
@@ -1187,7 +1187,9 @@ int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i
     if (sums_out == nullptr) {
       RSC_CUDA(cudaMemsetAsync(w, 0, 4 * gsz + 2 * asz + sizeof(FusedPlan), st));
     } else {
-      RSC_CUDA(cudaMemsetAsync(sums_out, 0, 4 * sizeof(double) * G, st));
+      // only the requested sets are written (rsc.h): a caller may keep another set's sums here
+      if (which & RSC_MOMENTS_LOG) RSC_CUDA(cudaMemsetAsync(sums_out, 0, 2 * sizeof(double) * G, st));
+      if (which & RSC_MOMENTS_LIN) RSC_CUDA(cudaMemsetAsync(sums_out + 2 * G, 0, 2 * sizeof(double) * G, st));
       RSC_CUDA(cudaMemsetAsync(accb, 0, 2 * asz + sizeof(FusedPlan), st));
     }
     if (row_splits == nullptr) {

@@ -463,7 +463,7 @@ int launch_qc(const rsc_csr& X, const uint8_t* gene_flags, int64_t* cell_total_i
   while (a.check_shift < 9u && (2u << a.check_shift) <= (uint32_t)g_opt.qc_row_budget) ++a.check_shift;
   a.flush_all = g_opt.flush_all ? 1u : 0u;
   int64_t blocks = (X.n_rows + kQcWarps * kQcRowsPerGrab - 1) / (kQcWarps * kQcRowsPerGrab);
-  const int cap = g_opt.grid_ctas > 0 ? g_opt.grid_ctas : sm_count();
+  const int cap = g_opt.grid_ctas.load() > 0 ? g_opt.grid_ctas.load() : sm_count();
   if (blocks > cap) blocks = cap;
   // in-stream counting serves a list {0, k1 < .. < kNB, K} with 1 <= NB <= 3 interior entries
   int nb = 0;
