@@ -259,6 +259,34 @@ int rsc_hvg_cutoffs(int32_t n_genes, const double* mean_t, const double* disp_no
                     uint8_t* out_mask, int32_t* out_indices, int32_t* out_count, void* stream);
 
 /* ---------------------------------------------------------------------------------
+ * rsc_hvg_select_cell_ranger: cell-ranger-flavour HVG selection
+ * (reading R18) from the mean / variance of the NORMALISED, non-logged
+ * matrix (mean_lin / var_lin of rsc_normalize_log1p_moments):
+ *   mean == 0 -> 1e-12; d = var / mean; bins = the intervals (e_k, e_{k+1}] of the edges -inf, P10,
+ *   P15, .., P100 of the means (linear interpolation; equal edges merged), +inf;
+ *   z = (d - median_bin(d)) / (median_bin |d - median_bin(d)| / 0.6745)  (IEEE: a zero MAD gives
+ *   +-inf or NaN); cutoff = n_top-th largest non-NaN z; mask = z >= cutoff.
+ *   Outputs as rsc_hvg_select (out_disp, out_disp_norm, out_bin, out_indices optional).
+ *   1 <= n_genes <= 65 535, n_top >= 1.
+ *
+ * rsc_hvg_merge_batches: per-batch HVG (reading R19): the selection was run once per batch of cells
+ * (row ranges of the matrix; any flavour); masks uint8[n_batches][n_genes] and disp_norm
+ * double[n_batches][n_genes] hold its per-batch outputs.  Per gene: out_nbatches = number of
+ * batches that selected it, out_disp_norm_mean = mean of its non-NaN normalised dispersions (NaN
+ * if none); genes are ranked by (nbatches, mean dispersion) descending, NaN last inside a level,
+ * and every gene at or above the n_top-th is selected.  1 <= n_batches <= 256.
+ * ------------------------------------------------------------------------------- */
+size_t rsc_hvg_select_cell_ranger_workspace_bytes(int32_t n_genes);
+int rsc_hvg_select_cell_ranger(int32_t n_genes, const double* gene_mean, const double* gene_var,
+                               int32_t n_top, double* out_disp, double* out_disp_norm,
+                               int32_t* out_bin, uint8_t* out_mask, int32_t* out_indices,
+                               int32_t* out_count, void* ws, size_t ws_bytes, void* stream);
+int rsc_hvg_merge_batches(int32_t n_genes, int32_t n_batches, const uint8_t* masks,
+                          const double* disp_norm, int32_t n_top, int32_t* out_nbatches,
+                          double* out_disp_norm_mean, uint8_t* out_mask, int32_t* out_indices,
+                          int32_t* out_count, void* stream);
+
+/* ---------------------------------------------------------------------------------
  * SURVEY.md 8(f) NEXT-3 (first half) -- rsc_scale_dense: z-score per gene with optional clip
  * ("scaling"), written as a DENSE row-major float32 [n_rows, n_cols] matrix
  * (run it after subsetting to the HVGs: the output has n_rows * n_cols elements):

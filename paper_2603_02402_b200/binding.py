@@ -42,6 +42,7 @@ EXPORTS = [
     "rsc_filter_masks", "rsc_subset_csr_workspace_bytes", "rsc_subset_csr_plan", "rsc_subset_csr_fill",
     "rsc_scale_dense_workspace_bytes", "rsc_scale_dense", "rsc_hvg_cutoffs",
     "rsc_gram_cov_workspace_bytes", "rsc_gram_cov",
+    "rsc_hvg_select_cell_ranger_workspace_bytes", "rsc_hvg_select_cell_ranger", "rsc_hvg_merge_batches",
     "rsc_preprocess_workspace_bytes", "rsc_preprocess",
     "rsc_preprocess_host_workspace_bytes", "rsc_preprocess_host",
 ]
@@ -109,6 +110,9 @@ def lib() -> C.CDLL:
     L.rsc_hvg_select_workspace_bytes.argtypes = [i32, i32]
     L.rsc_subset_csr_workspace_bytes.argtypes = [i64, i32]
     L.rsc_scale_dense_workspace_bytes.argtypes = [i32]
+    L.rsc_hvg_select_cell_ranger_workspace_bytes.argtypes = [i32]
+    L.rsc_hvg_select_cell_ranger.argtypes = [i32, p, p, i32, p, p, p, p, p, p, p, sz, p]
+    L.rsc_hvg_merge_batches.argtypes = [i32, i32, p, p, i32, p, p, p, p, p, p]
     L.rsc_gram_cov_workspace_bytes.argtypes = [i64, i32, i64]
     L.rsc_gram_cov.argtypes = [p, p, p, p, p, sz, p]
     L.rsc_hvg_cutoffs.argtypes = [i32, p, p, C.c_double, C.c_double, C.c_double, C.c_double, p, p, p, p]
@@ -542,6 +546,74 @@ def rsc_scale_dense(X: Csr, gene_mean: torch.Tensor, gene_var: torch.Tensor,
 
 
 # --------------------------------------------------------------------------- NEXT-4 (part): cutoffs
+def rsc_hvg_select_cell_ranger(gene_mean: torch.Tensor, gene_var: torch.Tensor, n_top: int, stream=None) -> dict:
+    """Cell-ranger-flavour HVG selection from the moments of the normalised, non-logged matrix."""
+    if not gene_mean.is_cuda:
+        raise RscError(RSC_ERR_INVALID_ARG, "device tensors required (no CPU fallback)")
+    assert gene_mean.dtype == torch.float64 and gene_var.dtype == torch.float64
+    L, dev, G = lib(), gene_mean.device, gene_mean.shape[0]
+    out = dict(disp=torch.empty(G, dtype=torch.float64, device=dev),
+               disp_norm=torch.empty(G, dtype=torch.float64, device=dev),
+               bin=torch.empty(G, dtype=torch.int32, device=dev),
+               mask=torch.empty(G, dtype=torch.uint8, device=dev),
+               indices=torch.full((G,), -1, dtype=torch.int32, device=dev),
+               count=torch.zeros(1, dtype=torch.int32, device=dev))
+    ws = _ws(L.rsc_hvg_select_cell_ranger_workspace_bytes(G), dev, stream)
+    _check(L.rsc_hvg_select_cell_ranger(G, _ptr(gene_mean), _ptr(gene_var), n_top, _ptr(out["disp"]),
+                                        _ptr(out["disp_norm"]), _ptr(out["bin"]), _ptr(out["mask"]),
+                                        _ptr(out["indices"]), _ptr(out["count"]), _ptr(ws), ws.numel(),
+                                        _stream(stream)))
+    return out
+
+
+def rsc_hvg_merge_batches(masks: torch.Tensor, disp_norm: torch.Tensor, n_top: int, stream=None) -> dict:
+    """Merge per-batch HVG selections: masks uint8 [B, G], disp_norm float64 [B, G] (device)."""
+    if not masks.is_cuda:
+        raise RscError(RSC_ERR_INVALID_ARG, "device tensors required (no CPU fallback)")
+    assert masks.dtype == torch.uint8 and disp_norm.dtype == torch.float64
+    assert masks.is_contiguous() and disp_norm.is_contiguous() and masks.shape == disp_norm.shape
+    Bn, G = masks.shape
+    dev = masks.device
+    out = dict(nbatches=torch.empty(G, dtype=torch.int32, device=dev),
+               disp_norm_mean=torch.empty(G, dtype=torch.float64, device=dev),
+               mask=torch.empty(G, dtype=torch.uint8, device=dev),
+               indices=torch.full((G,), -1, dtype=torch.int32, device=dev),
+               count=torch.zeros(1, dtype=torch.int32, device=dev))
+    _check(lib().rsc_hvg_merge_batches(G, Bn, _ptr(masks), _ptr(disp_norm), n_top, _ptr(out["nbatches"]),
+                                       _ptr(out["disp_norm_mean"]), _ptr(out["mask"]), _ptr(out["indices"]),
+                                       _ptr(out["count"]), _stream(stream)))
+    return out
+
+
+def rsc_hvg_select_batched(X: Csr, batch_offsets, gene_flags, target_sum: float, n_top: int, n_bins: int = 20,
+                           flavor: str = "seurat") -> dict:
+    """Per-batch HVG over contiguous row ranges (batch b = rows batch_offsets[b] .. batch_offsets[b+1]):
+    the chain runs once per batch on its row slice (x'' is written in place, so afterwards the whole
+    matrix is log-normalised), the per-batch selections are merged by rsc_hvg_merge_batches.
+    Marshalling only: every step is a C-ABI call."""
+    _need_cuda(X)
+    nb = len(batch_offsets) - 1
+    masks = torch.empty(nb, X.n_cols, dtype=torch.uint8, device=X.device)
+    zs = torch.empty(nb, X.n_cols, dtype=torch.float64, device=X.device)
+    per_batch = []
+    for b in range(nb):
+        r0, r1 = int(batch_offsets[b]), int(batch_offsets[b + 1])
+        p0, p1 = int(X.indptr[r0]), int(X.indptr[r1])
+        Xb = Csr((X.indptr[r0:r1 + 1] - p0).contiguous(), X.indices[p0:p1], X.data[p0:p1], X.n_cols,
+                 X.sorted_indices)
+        o = rsc_preprocess(Xb, gene_flags, target_sum, n_top, n_bins, which_moments=RSC_MOMENTS_LOG | RSC_MOMENTS_LIN,
+                           hvg_on_linear=True)
+        if flavor == "cell_ranger":
+            h = rsc_hvg_select_cell_ranger(o["mean_lin"], o["var_lin"], n_top)
+            masks[b].copy_(h["mask"]); zs[b].copy_(h["disp_norm"])
+        else:
+            masks[b].copy_(o["hvg_mask"]); zs[b].copy_(o["hvg_disp_norm"])
+        per_batch.append(o)
+    out = rsc_hvg_merge_batches(masks, zs, n_top)
+    out["batch_masks"], out["batch_disp_norm"], out["per_batch"] = masks, zs, per_batch
+    return out
+
+
 def rsc_gram_cov(X: Csr, want_gram: bool = True, want_cov: bool = True, stream=None) -> dict:
     """PAPER.md:L95 mu, S = X^T X, C = (S - n mu mu^T) / (n - 1) on the tensor cores (float64 outputs)."""
     _need_cuda(X)

@@ -318,6 +318,37 @@ int rsc_hvg_cutoffs(int32_t n_genes, const double* mean_t, const double* disp_no
                             out_indices, out_count, static_cast<cudaStream_t>(stream));
 }
 
+size_t rsc_hvg_select_cell_ranger_workspace_bytes(int32_t n_genes) { return hvg_cell_ranger_workspace_bytes(n_genes); }
+
+int rsc_hvg_select_cell_ranger(int32_t n_genes, const double* gene_mean, const double* gene_var, int32_t n_top,
+                               double* out_disp, double* out_disp_norm, int32_t* out_bin, uint8_t* out_mask,
+                               int32_t* out_indices, int32_t* out_count, void* ws, size_t ws_bytes, void* stream) {
+  RSC_CHECK_ARG(n_genes >= 1 && n_genes <= 65535, "rsc_hvg_select_cell_ranger: n_genes must be in [1, 65535]");
+  RSC_CHECK_ARG(gene_mean != nullptr && gene_var != nullptr, "rsc_hvg_select_cell_ranger: mean / var is NULL");
+  RSC_CHECK_ARG(n_top >= 1, "rsc_hvg_select_cell_ranger: n_top < 1");
+  RSC_CHECK_ARG(out_mask != nullptr && out_count != nullptr, "rsc_hvg_select_cell_ranger: out_mask / out_count is NULL");
+  int rc = check_device();
+  if (rc) return rc;
+  if ((rc = check_ws("rsc_hvg_select_cell_ranger", ws, ws_bytes, hvg_cell_ranger_workspace_bytes(n_genes)))) return rc;
+  return launch_hvg_cell_ranger(n_genes, gene_mean, gene_var, n_top, out_disp, out_disp_norm, out_bin, out_mask,
+                                out_indices, out_count, ws, static_cast<cudaStream_t>(stream));
+}
+
+int rsc_hvg_merge_batches(int32_t n_genes, int32_t n_batches, const uint8_t* masks, const double* disp_norm,
+                          int32_t n_top, int32_t* out_nbatches, double* out_disp_norm_mean, uint8_t* out_mask,
+                          int32_t* out_indices, int32_t* out_count, void* stream) {
+  RSC_CHECK_ARG(n_genes >= 1, "rsc_hvg_merge_batches: n_genes < 1");
+  RSC_CHECK_ARG(n_batches >= 1 && n_batches <= 256, "rsc_hvg_merge_batches: n_batches must be in [1, 256]");
+  RSC_CHECK_ARG(masks != nullptr && disp_norm != nullptr, "rsc_hvg_merge_batches: masks / disp_norm is NULL");
+  RSC_CHECK_ARG(n_top >= 1, "rsc_hvg_merge_batches: n_top < 1");
+  RSC_CHECK_ARG(out_nbatches != nullptr && out_disp_norm_mean != nullptr && out_mask != nullptr && out_count != nullptr,
+                "rsc_hvg_merge_batches: a required output is NULL");
+  int rc = check_device();
+  if (rc) return rc;
+  return launch_hvg_merge_batches(n_genes, n_batches, masks, disp_norm, n_top, out_nbatches, out_disp_norm_mean,
+                                  out_mask, out_indices, out_count, static_cast<cudaStream_t>(stream));
+}
+
 size_t rsc_gram_cov_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz) {
   return gram_workspace_bytes(n_rows, n_cols, nnz);
 }
