@@ -453,6 +453,14 @@ def main():
                          "peak_source": peak_src + " bf16_tflops (burst); fp16 = bf16 rate (guide's nominal ratio 1)",
                          "flops": "3 n p^2: hi*hi + hi*lo + lo*hi on the upper triangle; tile padding not counted"},
             "note": "whole rsc_gram_cov call: exact mean (moments pass), pack to fp16 hi/lo planes, MMA, finalize"}
+        # the projection of L95 on 50 loadings (orthonormal random V: the eigensolver is a library call)
+        Vq = torch.linalg.qr(torch.randn(g2, 50, dtype=torch.float64, device=dev))[0].contiguous()
+        mu64 = out_h["mean_log"][sel].contiguous()
+        ms, Zp = timed(torch, lambda: binding.rsc_pca_transform(Y, Vq, mu64), reps=3, warm=2)
+        del Zp, Vq
+        nxt["pca_transform (HVG columns, 50 components)"] = {
+            "ms": ms, "GBps_L2_table_reads": 200.0 * Y.nnz / (ms / 1e3) / 1e9,
+            "note": "Z = XV - 1 mu^T V; a 200-byte row of the float32 V table per stored entry (L2 / L1), fp64 accumulation"}
         del Y, q
 
     # ---- end to end through the host entry point (rank-local; N=1 only)

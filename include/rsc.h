@@ -259,6 +259,20 @@ int rsc_hvg_cutoffs(int32_t n_genes, const double* mean_t, const double* disp_no
                     uint8_t* out_mask, int32_t* out_indices, int32_t* out_count, void* stream);
 
 /* ---------------------------------------------------------------------------------
+ * rsc_pca_transform -- PAPER.md:L95 "The sparse-to-dense transform applies implicit centering in
+ * chunks: Z = XV - 1 (mu^T V)": the projection of the cells on k loadings (the eigenvectors of C,
+ * computed by the caller's eigensolver -- a library call, out of scope here).
+ *   V: double[n_cols][n_comps] row-major; gene_mean: double[n_cols] (out_mean of rsc_gram_cov) or
+ *   NULL (no centring: the uncentred truncated-SVD projection the paper also provides);
+ *   out: float[n_rows][n_comps].  Products are accumulated in double from a float32 copy of V
+ *   (|Z - Z_exact| <= 1e-7 * sum_j |x_ij V_jc| + float32 rounding of the result).
+ *   1 <= n_comps <= 128.  ws: rsc_pca_transform_workspace_bytes(n_cols, n_comps).
+ * ------------------------------------------------------------------------------- */
+size_t rsc_pca_transform_workspace_bytes(int32_t n_cols, int32_t n_comps);
+int rsc_pca_transform(const rsc_csr* X, const double* V, const double* gene_mean, int32_t n_comps,
+                      float* out, void* ws, size_t ws_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------
  * rsc_hvg_select_cell_ranger: cell-ranger-flavour HVG selection
  * (reading R18) from the mean / variance of the NORMALISED, non-logged
  * matrix (mean_lin / var_lin of rsc_normalize_log1p_moments):

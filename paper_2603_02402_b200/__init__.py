@@ -12,13 +12,13 @@ from .binding import (  # noqa: F401
     RSC_CSR_SORTED, RSC_HVG_SEURAT_LOG, RSC_MOMENTS_LIN, RSC_MOMENTS_LOG,
     rsc_gene_moments, rsc_hvg_select, rsc_log1p, rsc_moments_finalize, rsc_normalize_log1p_moments,
     rsc_normalize_total, rsc_preprocess, rsc_qc_metrics, rsc_version,
-    rsc_filter_masks, rsc_subset_csr, rsc_scale_dense, rsc_gram_cov,
+    rsc_filter_masks, rsc_subset_csr, rsc_scale_dense, rsc_gram_cov, rsc_pca_transform,
     rsc_hvg_select_cell_ranger, rsc_hvg_merge_batches, rsc_hvg_select_batched, rsc_hvg_cutoffs,
 )
 
 __all__ = [
     "Csr", "HostPreprocessor", "Preprocessor", "RscError", "rsc_gene_moments", "rsc_hvg_select",
     "rsc_log1p", "rsc_moments_finalize", "rsc_normalize_log1p_moments", "rsc_normalize_total", "rsc_preprocess",
-    "rsc_qc_metrics", "rsc_version", "rsc_filter_masks", "rsc_subset_csr", "rsc_scale_dense", "rsc_gram_cov",
+    "rsc_qc_metrics", "rsc_version", "rsc_filter_masks", "rsc_subset_csr", "rsc_scale_dense", "rsc_gram_cov", "rsc_pca_transform",
     "rsc_hvg_select_cell_ranger", "rsc_hvg_merge_batches", "rsc_hvg_select_batched", "rsc_hvg_cutoffs",
 ]

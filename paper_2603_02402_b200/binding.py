@@ -41,7 +41,7 @@ EXPORTS = [
     "rsc_hvg_select_workspace_bytes", "rsc_hvg_select",
     "rsc_filter_masks", "rsc_subset_csr_workspace_bytes", "rsc_subset_csr_plan", "rsc_subset_csr_fill",
     "rsc_scale_dense_workspace_bytes", "rsc_scale_dense", "rsc_hvg_cutoffs",
-    "rsc_gram_cov_workspace_bytes", "rsc_gram_cov",
+    "rsc_gram_cov_workspace_bytes", "rsc_gram_cov", "rsc_pca_transform_workspace_bytes", "rsc_pca_transform",
     "rsc_hvg_select_cell_ranger_workspace_bytes", "rsc_hvg_select_cell_ranger", "rsc_hvg_merge_batches",
     "rsc_preprocess_workspace_bytes", "rsc_preprocess",
     "rsc_preprocess_host_workspace_bytes", "rsc_preprocess_host",
@@ -113,6 +113,8 @@ def lib() -> C.CDLL:
     L.rsc_hvg_select_cell_ranger_workspace_bytes.argtypes = [i32]
     L.rsc_hvg_select_cell_ranger.argtypes = [i32, p, p, i32, p, p, p, p, p, p, p, sz, p]
     L.rsc_hvg_merge_batches.argtypes = [i32, i32, p, p, i32, p, p, p, p, p, p]
+    L.rsc_pca_transform_workspace_bytes.argtypes = [i32, i32]
+    L.rsc_pca_transform.argtypes = [p, p, p, i32, p, p, sz, p]
     L.rsc_gram_cov_workspace_bytes.argtypes = [i64, i32, i64]
     L.rsc_gram_cov.argtypes = [p, p, p, p, p, sz, p]
     L.rsc_hvg_cutoffs.argtypes = [i32, p, p, C.c_double, C.c_double, C.c_double, C.c_double, p, p, p, p]
@@ -611,6 +613,21 @@ def rsc_hvg_select_batched(X: Csr, batch_offsets, gene_flags, target_sum: float,
         per_batch.append(o)
     out = rsc_hvg_merge_batches(masks, zs, n_top)
     out["batch_masks"], out["batch_disp_norm"], out["per_batch"] = masks, zs, per_batch
+    return out
+
+
+def rsc_pca_transform(X: Csr, V: torch.Tensor, gene_mean: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """PAPER.md:L95 Z = X V - 1 (mu^T V) as float32 [n_rows, n_comps]; V float64 [n_cols, n_comps]."""
+    _need_cuda(X)
+    assert V.is_cuda and V.dtype == torch.float64 and V.is_contiguous() and V.shape[0] == X.n_cols
+    assert gene_mean is None or (gene_mean.dtype == torch.float64 and gene_mean.is_cuda)
+    k = int(V.shape[1])
+    out = torch.empty(X.n_rows, k, dtype=torch.float32, device=X.device)
+    L = lib()
+    ws = _ws(L.rsc_pca_transform_workspace_bytes(X.n_cols, k), X.device, stream)
+    cs = X.c_struct()
+    _check(L.rsc_pca_transform(C.byref(cs), _ptr(V), _ptr(gene_mean), k, _ptr(out), _ptr(ws), ws.numel(),
+                               _stream(stream)))
     return out
 
 

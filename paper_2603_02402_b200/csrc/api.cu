@@ -349,6 +349,20 @@ int rsc_hvg_merge_batches(int32_t n_genes, int32_t n_batches, const uint8_t* mas
                                   out_mask, out_indices, out_count, static_cast<cudaStream_t>(stream));
 }
 
+size_t rsc_pca_transform_workspace_bytes(int32_t n_cols, int32_t n_comps) { return pca_workspace_bytes(n_cols, n_comps); }
+
+int rsc_pca_transform(const rsc_csr* X, const double* V, const double* gene_mean, int32_t n_comps, float* out,
+                      void* ws, size_t ws_bytes, void* stream) {
+  int rc = check_csr(X, "rsc_pca_transform", true);
+  if (rc) return rc;
+  RSC_CHECK_ARG(pca_supported(n_comps), "rsc_pca_transform: n_comps must be in [1, 128]");
+  RSC_CHECK_ARG(V != nullptr, "rsc_pca_transform: V is NULL");
+  RSC_CHECK_ARG(out != nullptr || X->n_rows == 0, "rsc_pca_transform: out is NULL");
+  if ((rc = check_device())) return rc;
+  if ((rc = check_ws("rsc_pca_transform", ws, ws_bytes, pca_workspace_bytes(X->n_cols, n_comps)))) return rc;
+  return launch_pca_transform(*X, V, gene_mean, n_comps, out, ws, static_cast<cudaStream_t>(stream));
+}
+
 size_t rsc_gram_cov_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz) {
   return gram_workspace_bytes(n_rows, n_cols, nnz);
 }

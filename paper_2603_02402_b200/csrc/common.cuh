@@ -127,6 +127,10 @@ int launch_hvg_cell_ranger(int32_t G, const double* mean, const double* var, int
 int launch_hvg_merge_batches(int32_t G, int32_t B, const uint8_t* masks, const double* disp_norm, int32_t n_top,
                              int32_t* out_nbatches, double* out_mean, uint8_t* out_mask, int32_t* out_idx,
                              int32_t* out_count, cudaStream_t st);
+size_t pca_workspace_bytes(int32_t n_cols, int32_t n_comps);
+bool pca_supported(int32_t n_comps);
+int launch_pca_transform(const rsc_csr& X, const double* V, const double* mean, int32_t k, float* out, void* ws,
+                         cudaStream_t st);
 size_t gram_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
 bool gram_supported(int32_t n_cols);
 int launch_gram_cov(const rsc_csr& X, double* out_mean, double* out_gram, double* out_cov, void* ws,

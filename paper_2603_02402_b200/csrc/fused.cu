@@ -66,7 +66,10 @@ constexpr long long kCheckBit = 1LL << 62;  // set in a grab's result: this grab
 constexpr int kMaxGroups = 64;
 // rows a CTA can add between two checks of a gene: the check interval (<= 512) + the grabs its
 // warps hold (current, next, pending) must stay below kMaxRowsBetweenChecks (see check_tables)
-constexpr int kCheckRows = 256;            // default / largest check interval
+#ifndef RSC_FU_CHECK
+#define RSC_FU_CHECK 256
+#endif
+constexpr int kCheckRows = RSC_FU_CHECK;   // default / largest check interval (a power of two)
 constexpr int kMaxRowsBetweenChecks = 410;
 static_assert(kCheckRows + 3 * (kFuThreads / 32) * kFuRowsPerGrab + 16 <= kMaxRowsBetweenChecks,
               "fused pass: too many rows in flight for the lazy flush");
@@ -1205,7 +1208,7 @@ int launch_fused(const rsc_csr& X, float target_sum, const int64_t* cell_total_i
     a.splits = row_splits; a.target_sum = target_sum;
     a.row_budget = 4000u;
     a.check_shift = 0u;                                         // largest power of two <= the option (<= 512)
-    while (a.check_shift < 8u && (2u << a.check_shift) <= (uint32_t)g_opt.fused_row_budget) ++a.check_shift;
+    while ((2u << a.check_shift) <= (uint32_t)kCheckRows && (2u << a.check_shift) <= (uint32_t)g_opt.fused_row_budget) ++a.check_shift;
     a.flush_all = g_opt.flush_all ? 1u : 0u;
     a.S1log = S1log; a.S2log = S2log; a.S1lin = S1lin; a.S2lin = S2lin; a.plan = plan;
     const bool int_acc = !(which & RSC_MOMENTS_FP64_ACC);
@@ -1304,7 +1307,7 @@ int launch_moments_fast(const rsc_csr& X, int ddof, double* mean, double* var, d
   a.indptr = X.indptr; a.indices = X.indices; a.data = X.data; a.cell_total = nullptr;
   a.splits = splits; a.target_sum = 1.0f; a.row_budget = 0u;
   a.check_shift = 0u;
-  while (a.check_shift < 8u && (2u << a.check_shift) <= (uint32_t)g_opt.fused_row_budget) ++a.check_shift;
+  while ((2u << a.check_shift) <= (uint32_t)kCheckRows && (2u << a.check_shift) <= (uint32_t)g_opt.fused_row_budget) ++a.check_shift;
   a.flush_all = g_opt.flush_all ? 1u : 0u;
   a.S1log = S1; a.S2log = S2; a.S1lin = S1; a.S2lin = S2; a.plan = plan;
   a.acc_log = reinterpret_cast<unsigned long long*>(accb);

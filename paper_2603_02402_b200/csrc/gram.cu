@@ -564,3 +564,107 @@ int launch_gram_cov(const rsc_csr& X, double* out_mean, double* out_gram, double
 bool gram_supported(int32_t n_cols) { return n_cols >= 1 && n_cols <= kGmMaxCols; }
 
 }  // namespace rsc
+
+// ------------------------------------------------------------------ PCA projection
+// Z = X V - 1 (mu^T V): "the sparse-to-dense transform applies implicit centering": a warp per cell,
+// lanes over the components; every stored entry adds x * V[gene][:] (V as a float32 table that
+// stays in L2 / L1: p x k x 4 B), accumulated in double, minus the per-component shift mu^T V.
+namespace rsc {
+
+constexpr int kPcaMaxComps = 128;
+
+__global__ void __launch_bounds__(256)
+pca_prep_kernel(int32_t p, int32_t k, int32_t kp, const double* __restrict__ V, const double* __restrict__ mean,
+                float* __restrict__ Vf, double* __restrict__ shift) {
+  // block c < k: shift[c] = sum_j mean_j V[j][c]; all blocks: their slice of the float table
+  const int tid = threadIdx.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + tid; i < (int64_t)p * kp; i += (int64_t)gridDim.x * blockDim.x) {
+    const int j = (int)(i / kp), c = (int)(i - (int64_t)j * kp);
+    Vf[i] = c < k ? (float)V[(size_t)j * k + c] : 0.0f;
+  }
+  __shared__ double red[8];
+  for (int c = blockIdx.x; c < k; c += gridDim.x) {
+    double s = 0.0;
+    if (mean != nullptr)
+      for (int j = tid; j < p; j += blockDim.x) s += mean[j] * V[(size_t)j * k + c];
+    s = warp_sum(s);
+    if ((tid & 31) == 0) red[tid >> 5] = s;
+    __syncthreads();
+    if (tid == 0) {
+      double t = 0.0;
+      for (int w = 0; w < 8; ++w) t += red[w];
+      shift[c] = t;
+    }
+    __syncthreads();
+  }
+}
+
+template <int KPL>
+__global__ void __launch_bounds__(256)
+pca_transform_kernel(int64_t n_rows, int32_t k, int32_t kp, const int64_t* __restrict__ indptr,
+                     const int32_t* __restrict__ indices, const float* __restrict__ data,
+                     const float* __restrict__ Vf, const double* __restrict__ shift, float* __restrict__ out) {
+  const int lane = threadIdx.x & 31;
+  const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  double sh[KPL];
+#pragma unroll
+  for (int c = 0; c < KPL; ++c) sh[c] = lane + 32 * c < k ? shift[lane + 32 * c] : 0.0;
+  for (int64_t row = warp0; row < n_rows; row += nwarps) {
+    const int64_t beg = indptr[row], end = indptr[row + 1];
+    double acc[KPL];
+#pragma unroll
+    for (int c = 0; c < KPL; ++c) acc[c] = 0.0;
+    for (int64_t p0 = beg; p0 < end; p0 += 32) {
+      const int64_t p = p0 + lane;
+      const int j = p < end ? __ldg(indices + p) : 0;
+      const float x = p < end ? __ldg(data + p) : 0.0f;
+      const int cnt = (int)min((int64_t)32, end - p0);
+      for (int t = 0; t < cnt; ++t) {
+        const int jj = __shfl_sync(0xffffffffu, j, t);
+        const double xx = (double)__shfl_sync(0xffffffffu, x, t);
+        const float* v = Vf + (size_t)jj * kp + lane;
+#pragma unroll
+        for (int c = 0; c < KPL; ++c) acc[c] = fma(xx, (double)__ldg(v + 32 * c), acc[c]);
+      }
+    }
+    float* o = out + row * (int64_t)k;
+#pragma unroll
+    for (int c = 0; c < KPL; ++c)
+      if (lane + 32 * c < k) o[lane + 32 * c] = (float)(acc[c] - sh[c]);
+  }
+}
+
+size_t pca_workspace_bytes(int32_t n_cols, int32_t n_comps) {
+  if (n_cols < 1 || n_comps < 1 || n_comps > kPcaMaxComps) return 0;
+  const size_t kp = (size_t)((n_comps + 31) / 32 * 32);
+  return align_up(sizeof(float) * (size_t)n_cols * kp, 256) + align_up(sizeof(double) * kPcaMaxComps, 256);
+}
+bool pca_supported(int32_t n_comps) { return n_comps >= 1 && n_comps <= kPcaMaxComps; }
+
+int launch_pca_transform(const rsc_csr& X, const double* V, const double* mean, int32_t k, float* out, void* ws,
+                         cudaStream_t st) {
+  if (X.n_rows == 0) return RSC_OK;
+  const int kp = (k + 31) / 32 * 32;
+  unsigned char* w = static_cast<unsigned char*>(ws);
+  float* Vf = reinterpret_cast<float*>(w);
+  double* shift = reinterpret_cast<double*>(w + align_up(sizeof(float) * (size_t)X.n_cols * kp, 256));
+  int64_t pb = ((int64_t)X.n_cols * kp + 255) / 256;
+  if (pb < k) pb = k;
+  if (pb > 4096) pb = 4096;
+  pca_prep_kernel<<<(unsigned)pb, 256, 0, st>>>(X.n_cols, k, kp, V, mean, Vf, shift);
+  RSC_LAUNCH_CHECK("pca_prep_kernel");
+  int64_t blocks = (X.n_rows + 7) / 8;
+  const int64_t cap = (int64_t)sm_count() * 8;
+  if (blocks > cap) blocks = cap;
+  switch (kp / 32) {
+    case 1: pca_transform_kernel<1><<<(unsigned)blocks, 256, 0, st>>>(X.n_rows, k, kp, X.indptr, X.indices, X.data, Vf, shift, out); break;
+    case 2: pca_transform_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(X.n_rows, k, kp, X.indptr, X.indices, X.data, Vf, shift, out); break;
+    case 3: pca_transform_kernel<3><<<(unsigned)blocks, 256, 0, st>>>(X.n_rows, k, kp, X.indptr, X.indices, X.data, Vf, shift, out); break;
+    default: pca_transform_kernel<4><<<(unsigned)blocks, 256, 0, st>>>(X.n_rows, k, kp, X.indptr, X.indices, X.data, Vf, shift, out); break;
+  }
+  RSC_LAUNCH_CHECK("pca_transform_kernel");
+  return RSC_OK;
+}
+
+}  // namespace rsc

@@ -69,3 +69,36 @@ def test_gram_cov_hvg_subset_of_cfg1():
     torch.cuda.synchronize()
     ip, ix, dl = Y.indptr.cpu().numpy(), Y.indices.cpu().numpy(), Y.data.cpu().numpy()
     _check(ip, ix, dl, g2)
+
+
+@pytest.mark.parametrize("n,G,k,seed,center", [(300, 100, 5, 0, True), (1000, 300, 50, 1, True), (777, 129, 33, 2, False),
+                                               (2000, 500, 128, 3, True), (64, 40, 1, 4, True)])
+def test_pca_transform(n, G, k, seed, center):
+    """rsc_pca_transform against oracle_np.pca_transform (PAPER.md:L95 Z = XV - 1 mu^T V).  Bound: V
+    travels as float32 (6e-8 per term) and the result is rounded to float32."""
+    ip, ix, dl = _log_csr(n, G, seed, 1.0)
+    rng = np.random.default_rng(seed)
+    V = np.linalg.qr(rng.standard_normal((G, k)))[0] if k <= G else rng.standard_normal((G, k))
+    V = np.ascontiguousarray(V)
+    X = Csr(torch.from_numpy(ip).cuda(), torch.from_numpy(ix).cuda(), torch.from_numpy(dl).cuda(), G)
+    dense = np.zeros((n, G)); dense[np.repeat(np.arange(n), np.diff(ip)), ix] = dl
+    mu = dense.mean(axis=0)
+    Z = B.rsc_pca_transform(X, torch.from_numpy(V).cuda(), torch.from_numpy(mu).cuda() if center else None)
+    torch.cuda.synchronize()
+    ref = O.pca_transform(ip, ix, dl, G, V, mu if center else np.zeros(G))
+    mass = np.abs(dense) @ np.abs(V) + (np.abs(mu) @ np.abs(V))[None, :] * (1 if center else 0)
+    err = np.abs(Z.cpu().numpy() - ref)
+    assert np.all(err <= 1e-7 * mass + 1.2e-7 * np.abs(ref) + 1e-30), err.max()
+
+
+def test_gram_eigh_transform_workflow():
+    """Gram -> covariance -> eigenvectors (torch.linalg.eigh: the library step the paper also uses)
+    -> projection; the projected coordinates have the top eigenvalues as variances."""
+    ip, ix, dl = _log_csr(3000, 200, 7, 0.8)
+    X = Csr(torch.from_numpy(ip).cuda(), torch.from_numpy(ix).cuda(), torch.from_numpy(dl).cuda(), 200)
+    g = B.rsc_gram_cov(X)
+    w, U = torch.linalg.eigh(g["cov"])
+    V = U[:, -10:].contiguous()
+    Z = B.rsc_pca_transform(X, V, g["mean"]).double()
+    np.testing.assert_allclose(Z.var(dim=0, unbiased=True).cpu().numpy(), w[-10:].cpu().numpy(), rtol=2e-5)
+    assert float(Z.mean(dim=0).abs().max()) < 1e-5
