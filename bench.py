@@ -429,7 +429,8 @@ def main():
         for name, (ck, gk) in legs.items():
             del Y
             ms, (Y, g2) = timed(torch, lambda: binding.rsc_subset_csr(X, ck, gk), reps=4, warm=2)
-            byt = 4.0 * nnz + 8.0 * nnz + 8.0 * Y.nnz       # plan reads indices; fill reads both, writes kept
+            # plan reads indices (not when every column is kept: a pure row filter); fill reads both, writes kept
+            byt = (0.0 if g2 == X.n_cols else 4.0 * nnz) + 8.0 * nnz + 8.0 * Y.nnz
             nxt[name] = {"ms": ms, "nnz_out": Y.nnz, "n_rows_out": Y.n_rows, "n_cols_out": g2,
                          "GBps": byt / (ms / 1e3) / 1e9,
                          "note": "plan + size read-back + allocation + fill, CUDA events"}

@@ -62,6 +62,7 @@ struct SubsetWs {
   int64_t* row_off;          // [n_rows] offset of the row in the output (kept rows)
   uint32_t* row_cnt;         // [n_rows] kept entries of the row (0 for dropped rows)
   int64_t* blk;              // [2 * n_blocks] per scan block: kept rows, kept entries (then exclusive)
+  int64_t* meta;             // [3] copy of out_counts (kept rows, kept columns, kept entries) for the fill call
   size_t total;
 };
 
@@ -74,6 +75,7 @@ static SubsetWs carve_subset(void* ws, int64_t n_rows, int32_t n_cols) {
   w.row_off = reinterpret_cast<int64_t*>(b + o);  o += align_up(sizeof(int64_t) * (size_t)n_rows, 256);
   w.row_cnt = reinterpret_cast<uint32_t*>(b + o); o += align_up(sizeof(uint32_t) * (size_t)n_rows, 256);
   w.blk = reinterpret_cast<int64_t*>(b + o);      o += align_up(sizeof(int64_t) * 2 * (nb + 1), 256);
+  w.meta = reinterpret_cast<int64_t*>(b + o);     o += 256;
   w.total = o;
   return w;
 }
@@ -86,7 +88,7 @@ size_t subset_workspace_bytes(int64_t n_rows, int32_t n_cols) {
 // column map by one CTA: chunks of 1024 columns, ballot + warp counts, running base
 __global__ void __launch_bounds__(1024)
 subset_colmap_kernel(int32_t n_cols, const uint8_t* __restrict__ keep_cols, int32_t* __restrict__ col_map,
-                     int64_t* __restrict__ out_counts) {
+                     int64_t* __restrict__ out_counts, int64_t* __restrict__ meta) {
   __shared__ int wsum[32];
   __shared__ int s_base;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -105,17 +107,29 @@ subset_colmap_kernel(int32_t n_cols, const uint8_t* __restrict__ keep_cols, int3
     if (tid == 0) { int t = s_base; for (int w = 0; w < 32; ++w) t += wsum[w]; s_base = t; }
     __syncthreads();
   }
-  if (tid == 0) out_counts[1] = s_base;
+  if (tid == 0) { out_counts[1] = s_base; meta[1] = s_base; }
 }
 
-// kept entries per row (warp per row; dropped rows count 0)
+// kept entries per row (warp per row; dropped rows count 0).  When every column is kept (the
+// column map's kept count, already on the device, equals n_cols: a pure row filter) the count is
+// the row length and the indices are not read at all.  (128-bit quad loads were measured slower
+// than four independent 4-byte loads per lane here: the column-map gathers dominate.)
 __global__ void __launch_bounds__(256)
-subset_count_kernel(int64_t n_rows, const int64_t* __restrict__ indptr, const int32_t* __restrict__ indices,
-                    const uint8_t* __restrict__ keep_rows, const int32_t* __restrict__ col_map,
+subset_count_kernel(int64_t n_rows, int64_t nnz, int32_t n_cols, const int64_t* __restrict__ indptr,
+                    const int32_t* __restrict__ indices, const uint8_t* __restrict__ keep_rows,
+                    const int32_t* __restrict__ col_map, const int64_t* __restrict__ out_counts,
                     uint32_t* __restrict__ row_cnt) {
   const int lane = lane_id();
   const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  const bool all_cols = out_counts[1] == (int64_t)n_cols;
+  if (all_cols) {
+    for (int64_t row = warp0 * 32 + lane; row < n_rows; row += nwarps * 32) {
+      const bool k = keep_rows == nullptr || keep_rows[row] != 0;
+      row_cnt[row] = k ? (uint32_t)(indptr[row + 1] - indptr[row]) : 0u;
+    }
+    return;
+  }
   for (int64_t row = warp0; row < n_rows; row += nwarps) {
     unsigned c = 0;
     if (keep_rows == nullptr || keep_rows[row] != 0) {
@@ -211,18 +225,40 @@ subset_offsets_kernel(int64_t n_rows, const uint8_t* __restrict__ keep_rows,
 }
 
 // ------------------------------------------------------------------ subset: fill (warp per kept row)
+// Every column kept (pure row filter): the kept rows are copied as they are.  Otherwise an
+// ordered warp compaction (ballot prefix) through the column map.
 __global__ void __launch_bounds__(256)
-subset_fill_kernel(int64_t n_rows, const int64_t* __restrict__ indptr, const int32_t* __restrict__ indices,
-                   const float* __restrict__ data, const uint8_t* __restrict__ keep_rows,
-                   const int32_t* __restrict__ col_map, const int64_t* __restrict__ row_off,
+subset_fill_kernel(int64_t n_rows, int32_t n_cols, const int64_t* __restrict__ indptr,
+                   const int32_t* __restrict__ indices, const float* __restrict__ data,
+                   const uint8_t* __restrict__ keep_rows, const int32_t* __restrict__ col_map,
+                   const int64_t* __restrict__ row_off, const int64_t* __restrict__ out_counts,
                    int32_t* __restrict__ out_indices, float* __restrict__ out_data) {
   const int lane = lane_id();
   const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  const bool all_cols = out_counts[1] == (int64_t)n_cols;
   for (int64_t row = warp0; row < n_rows; row += nwarps) {
     if (keep_rows != nullptr && keep_rows[row] == 0) continue;
     const int64_t beg = indptr[row], end = indptr[row + 1];
     int64_t o = row_off[row];
+    if (all_cols) {
+      for (int64_t p0 = beg; p0 < end; p0 += 256) {       // 8 independent loads per lane and array in flight
+        int j[8];
+        float x[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          const int64_t p = p0 + u * 32 + lane;
+          j[u] = p < end ? __ldg(indices + p) : 0;
+          x[u] = p < end ? __ldg(data + p) : 0.0f;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          const int64_t p = p0 + u * 32 + lane;
+          if (p < end) { out_indices[o + (p - beg)] = j[u]; out_data[o + (p - beg)] = x[u]; }
+        }
+      }
+      continue;
+    }
     for (int64_t p0 = beg; p0 < end; p0 += 128) {         // 4 independent loads per lane in flight
       int j[4];
       float x[4];
@@ -251,7 +287,7 @@ subset_fill_kernel(int64_t n_rows, const int64_t* __restrict__ indptr, const int
 int launch_subset_plan(const rsc_csr& X, const uint8_t* keep_rows, const uint8_t* keep_cols,
                        int64_t* out_indptr, int64_t* out_counts, void* ws, cudaStream_t st) {
   SubsetWs w = carve_subset(ws, X.n_rows, X.n_cols);
-  subset_colmap_kernel<<<1, 1024, 0, st>>>(X.n_cols, keep_cols, w.col_map, out_counts);
+  subset_colmap_kernel<<<1, 1024, 0, st>>>(X.n_cols, keep_cols, w.col_map, out_counts, w.meta);
   RSC_LAUNCH_CHECK("subset_colmap_kernel");
   const int64_t n = X.n_rows;
   const int64_t nb = (n + kScanBlock - 1) / kScanBlock;
@@ -259,7 +295,8 @@ int launch_subset_plan(const rsc_csr& X, const uint8_t* keep_rows, const uint8_t
     int64_t blocks = (n + 7) / 8;
     const int64_t cap = (int64_t)sm_count() * 16;
     if (blocks > cap) blocks = cap;
-    subset_count_kernel<<<(unsigned)blocks, 256, 0, st>>>(n, X.indptr, X.indices, keep_rows, w.col_map, w.row_cnt);
+    subset_count_kernel<<<(unsigned)blocks, 256, 0, st>>>(n, X.nnz, X.n_cols, X.indptr, X.indices, keep_rows, w.col_map,
+                                                          w.meta, w.row_cnt);
     RSC_LAUNCH_CHECK("subset_count_kernel");
     subset_blocksum_kernel<<<(unsigned)nb, kScanBlock, 0, st>>>(n, keep_rows, w.row_cnt, w.blk);
     RSC_LAUNCH_CHECK("subset_blocksum_kernel");
@@ -279,8 +316,8 @@ int launch_subset_fill(const rsc_csr& X, const uint8_t* keep_rows, int32_t* out_
   int64_t blocks = (X.n_rows + 7) / 8;
   const int64_t cap = (int64_t)sm_count() * 16;
   if (blocks > cap) blocks = cap;
-  subset_fill_kernel<<<(unsigned)blocks, 256, 0, st>>>(X.n_rows, X.indptr, X.indices, X.data, keep_rows,
-                                                       w.col_map, w.row_off, out_indices, out_data);
+  subset_fill_kernel<<<(unsigned)blocks, 256, 0, st>>>(X.n_rows, X.n_cols, X.indptr, X.indices, X.data, keep_rows,
+                                                       w.col_map, w.row_off, w.meta, out_indices, out_data);
   RSC_LAUNCH_CHECK("subset_fill_kernel");
   return RSC_OK;
 }
