@@ -102,3 +102,28 @@ def test_gram_eigh_transform_workflow():
     Z = B.rsc_pca_transform(X, V, g["mean"]).double()
     np.testing.assert_allclose(Z.var(dim=0, unbiased=True).cpu().numpy(), w[-10:].cpu().numpy(), rtol=2e-5)
     assert float(Z.mean(dim=0).abs().max()) < 1e-5
+
+
+def test_gram_cov_many_slabs_and_wide():
+    """More cells than one pack / MMA slab (262 144): partial tiles accumulate across slabs; and
+    more genes than 16 column tiles.  Random sparse log-like values drawn directly (no NB)."""
+    rng = np.random.default_rng(11)
+    # (a) 300 000 cells x 64 genes, ~6 stored entries per cell
+    n, G = 300_000, 64
+    lens = rng.integers(0, 13, n)
+    ip = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    ix = np.concatenate([np.sort(rng.choice(G, l, replace=False)) for l in lens[:2000]] +
+                        [np.empty(0, dtype=np.int64)]).astype(np.int32)
+    # cheap generation for the bulk: the first 2000 rows' pattern repeats (rows stay canonical)
+    reps = -(-n // 2000)
+    lens2 = np.tile(lens[:2000], reps)[:n]
+    ip = np.concatenate([[0], np.cumsum(lens2)]).astype(np.int64)
+    ix = np.tile(ix, reps)[: ip[-1]].astype(np.int32)
+    dl = (0.3 + 3.0 * rng.random(ip[-1])).astype(np.float32)
+    _check(ip, ix, dl, G)
+    # (b) 1 200 cells x 4 500 genes (18 x 36 tiles, ragged last tiles)
+    n, G = 1200, 4500
+    dense = (rng.random((n, G)) < 0.03) * (0.3 + 3.0 * rng.random((n, G)))
+    r, c = np.nonzero(dense)
+    ip = np.concatenate([[0], np.cumsum(np.bincount(r, minlength=n))]).astype(np.int64)
+    _check(ip, c.astype(np.int32), dense[r, c].astype(np.float32), G)
