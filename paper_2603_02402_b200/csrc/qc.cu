@@ -153,57 +153,65 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
     }
   };
   auto opaque = [](int v) -> int { asm volatile("mov.u32 %0, %0;" : "+r"(v)); return v; };
-  // per-lane partial sums of the current row
-  unsigned t32, m32, n32;                               // fast path (counts <= 511)
+  // per-lane partial sums of the current row.  acc packs the fast path's two sums in one word,
+  // exactly as the table does: bits 0..19 the lane's total, bits 20..31 its detected-entry count
+  // (one add per entry).  A lane sees at most 57 840 / 32 = 1808 entries of a row (canonical CSR,
+  // n_cols <= kQcMaxGenes) of at most 511 each: 1808 * 511 < 2^20, so the fields cannot mix.
+  unsigned acc, m32;                                    // fast path (counts 1 .. 511)
   long long T64, M64;                                   // slow path (large / negative counts)
 
   // One quad of 4 consecutive entries.  EDGE: only entries e0 + k in [0, len) belong to the
   // row; the others add 0 to the spare word qsm[G].
+  // Fast path: every valid value truncates to an integer in 1 .. 511 (one unsigned compare on
+  // xi - 1 covers explicit zeros, fractions below 1, negatives and large counts): the word
+  // count | total = xi + 2^20 goes to the table with one atomic and to acc with one add; the
+  // flagged-subset sum is touched only when a returned word carries the flag bit (few genes).
   auto quad = [&](auto edge_tag, const int4 jv, const float4 xv, int e0, int len) {
     constexpr bool EDGE = decltype(edge_tag)::value;
     const int j[4] = {jv.x, jv.y, jv.z, jv.w};
     const float x[4] = {xv.x, xv.y, xv.z, xv.w};
     int xi[4];
-    bool valid[4];
-    bool slow = false;
+    unsigned worst = 0u;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-      valid[k] = !EDGE || (unsigned)(e0 + k) < (unsigned)len;
+      const bool valid = !EDGE || (unsigned)(e0 + k) < (unsigned)len;
       xi[k] = __float2int_rz(x[k]);
-      slow = slow || (valid[k] && (unsigned)xi[k] > kQcMaxFast);
+      const unsigned d = valid ? (unsigned)(xi[k] - 1) : 0u;
+      worst = max(worst, d);
     }
-    if (!slow) {
-      uint32_t old[4], xf[4];
+    if (worst < kQcMaxFast) {                           // all valid xi in 1 .. 511
+      uint32_t old[4], add[4];
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
-        const bool nz = valid[k] && x[k] != 0.0f;
-        xf[k] = valid[k] ? (uint32_t)xi[k] : 0u;
-        const uint32_t jj = valid[k] ? (uint32_t)j[k] : (uint32_t)G;
-        old[k] = qc_atoms_add(sbase + (jj << 2), xf[k] + (nz ? 0x100000u : 0u));
-        n32 += nz ? 1u : 0u;
-        t32 += xf[k];
+        const bool valid = !EDGE || (unsigned)(e0 + k) < (unsigned)len;
+        add[k] = valid ? (uint32_t)xi[k] + 0x100000u : 0u;
+        const uint32_t jj = valid ? (uint32_t)j[k] : (uint32_t)G;
+        old[k] = qc_atoms_add(sbase + (jj << 2), add[k]);
+        acc += add[k];
       }
+      if ((int)(old[0] | old[1] | old[2] | old[3]) < 0) {   // a flagged gene among the four (rare)
 #pragma unroll
-      for (int k = 0; k < 4; ++k) m32 += xf[k] & (uint32_t)((int)old[k] >> 31);
-    } else {                                            // rare: counts > 511, negative, non-finite
+        for (int k = 0; k < 4; ++k) m32 += (add[k] & 0xfffffu) & (uint32_t)((int)old[k] >> 31);
+      }
+    } else {                                            // rare: explicit zeros, fractions, counts > 511, negative, non-finite
 #pragma unroll 1
       for (int k = 0; k < 4; ++k) {
-        if (!valid[k]) continue;
+        if (EDGE && !((unsigned)(e0 + k) < (unsigned)len)) continue;
         const float xv1 = k == 0 ? x[0] : k == 1 ? x[1] : k == 2 ? x[2] : x[3];
         const int jj = k == 0 ? j[0] : k == 1 ? j[1] : k == 2 ? j[2] : j[3];
         const int xi1 = __float2int_rz(xv1);
+        const bool nz = xv1 != 0.0f;
         if ((unsigned)xi1 <= kQcMaxFast) {
-          const bool nz = xv1 != 0.0f;
-          const uint32_t o = qc_atoms_add(sbase + ((uint32_t)jj << 2), (uint32_t)xi1 + (nz ? 0x100000u : 0u));
-          n32 += nz ? 1u : 0u;
-          t32 += (uint32_t)xi1;
+          const uint32_t a1 = (uint32_t)xi1 + (nz ? 0x100000u : 0u);
+          const uint32_t o = qc_atoms_add(sbase + ((uint32_t)jj << 2), a1);
+          acc += a1;
           m32 += (uint32_t)xi1 & (uint32_t)((int)o >> 31);
         } else {
           const long long xl = (long long)xv1;
-          n32 += xv1 != 0.0f ? 1u : 0u;
+          acc += nz ? 0x100000u : 0u;
           T64 += xl;
           if (qsm[jj] >> 31) M64 += xl;
-          if (a.gene_n_cells != nullptr && xv1 != 0.0f) atomicAdd(&a.gene_n_cells[jj], 1);
+          if (a.gene_n_cells != nullptr && nz) atomicAdd(&a.gene_n_cells[jj], 1);
           if (xl != 0 && a.gene_total != nullptr)
             atomicAdd(&a.gene_total[jj], (unsigned long long)xl);
         }
@@ -241,7 +249,8 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
         const int head = (int)(beg - abeg);
         const int len = (int)(end - beg);
         const int span = opaque(len > 0 ? head + len : 0);
-        t32 = 0; m32 = 0; n32 = 0; T64 = 0; M64 = 0;
+        acc = 0; m32 = 0; T64 = 0; M64 = 0;
+        unsigned n32x = 0u;                               // NB = 1: the edge-step split count rides on the n_genes sum
         int cnt_i[NB > 0 ? NB : 1], cnt_e[NB > 0 ? NB : 1];   // entries below bound b: interior steps (warp-uniform) / edge steps (per lane)
 #pragma unroll
         for (int b = 0; b < NB; ++b) { cnt_i[b] = 0; cnt_e[b] = 0; }
@@ -313,7 +322,7 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
         if (SPLITS && NB > 0) {
           // cnt_i is stored complemented once the bound was crossed in an interior step.  NB = 1:
           // the edge-step count rides in the upper half of n32 (both < 2^16: n_cols < 57 841)
-          if (NB == 1) n32 += (unsigned)cnt_e[0] << 16;
+          if (NB == 1) n32x = (unsigned)cnt_e[0] << 16;
         } else if (SPLITS) {
           // split table of the row: lane k finds #{entries with column < k * RSC_SPLIT_WIDTH} by
           // binary search in the (sorted) row, whose lines were just streamed (L2 / L1 hits)
@@ -332,6 +341,8 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
             sp[k] = (uint32_t)lo;
           }
         }
+        const unsigned t32 = acc & 0xfffffu;
+        const unsigned n32 = (acc >> 20) + n32x;
         long long T, M;
         if (__any_sync(0xffffffffu, (T64 | M64) != 0)) {
           T = warp_sum_ll(T64 + (long long)t32);
