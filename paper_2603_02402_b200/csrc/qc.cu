@@ -36,6 +36,10 @@ constexpr int kQcRowsPerGrab = RSC_QC_RG;
 #define RSC_QC_AHEAD 4
 #endif
 constexpr int kQcAhead = RSC_QC_AHEAD;
+#ifndef RSC_QC_LONGROW
+#define RSC_QC_LONGROW 6144
+#endif
+constexpr int kQcLongRow = RSC_QC_LONGROW;       // entries: rows longer than this look one step less ahead
 #ifndef RSC_QC_EVICT
 #define RSC_QC_EVICT 0        // bit 0: demand loads carry L2 evict_first; bit 1: look-ahead prefetches carry evict_last
 #endif                  // L2 look-ahead of a warp, in steps of 128 entries
@@ -189,7 +193,10 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
         old[k] = qc_atoms_add(sbase + (jj << 2), add[k]);
         acc += add[k];
       }
-      if ((int)(old[0] | old[1] | old[2] | old[3]) < 0) {   // a flagged gene among the four (rare)
+#ifdef RSC_QC_FLAGBRANCH
+      if ((int)(old[0] | old[1] | old[2] | old[3]) < 0)   // a flagged gene among the four (rare)
+#endif
+      {
 #pragma unroll
         for (int k = 0; k < 4; ++k) m32 += (add[k] & 0xfffffu) & (uint32_t)((int)old[k] >> 31);
       }
@@ -282,7 +289,10 @@ __global__ void __launch_bounds__(kQcThreads, 1) qc_stream_kernel(const QcArgs a
         int4 jn = make_int4(0, 0, 0, 0);
         float4 xn = make_float4(0.f, 0.f, 0.f, 0.f);
         if (span > 0) load_q(ip, dp, e0, jn, xn);
-        int64_t pf = abeg + kQcAhead * 128;             // L2 look-ahead position (lane-uniform)
+        // L2 look-ahead position (lane-uniform): kQcAhead steps ahead, one step less inside long rows
+        // (measured: 4 steps serve ordinary rows best, cfg3 1.84 vs 1.87 ms with 3; the very long rows of
+        // cfg5's tail want 3: 1.97 vs 2.10 ms -- a longer distance costs DRAM re-reads there)
+        int64_t pf = abeg + (len > kQcLongRow ? kQcAhead - 1 : kQcAhead) * 128;
 #pragma unroll 2
         for (int base = 0; base < span; base += 128) {
           const int4 jc = jn;
