@@ -59,8 +59,12 @@ constexpr int kFuThreads = RSC_FU_THREADS;
 #endif
 constexpr int kFuRowsPerGrab = RSC_FU_RG;
 #ifndef RSC_FU_HEAD
-#define RSC_FU_HEAD 1024
+#define RSC_FU_HEAD 512
 #endif
+#ifndef RSC_FU_DIST
+#define RSC_FU_DIST RSC_FU_HEAD
+#endif
+constexpr int kFuDist = RSC_FU_DIST;          // in-segment look-ahead distance, entries (<= kFuHead)
 constexpr int kFuHead = RSC_FU_HEAD;              // entries of a segment requested from L2 before the segment is walked
 constexpr long long kCheckBit = 1LL << 62;  // set in a grab's result: this grab crossed a check point
 constexpr int kMaxGroups = 64;
@@ -845,11 +849,13 @@ __device__ __forceinline__ void fused_stream_body(const FusedArgs& a, uint32_t* 
         if (!MOM) ms = cell_scale(a.target_sum, a.cell_total[row]);
       }
     };
-    // L2 look-ahead.  The head of the NEXT segment (its first kFuHead entries: one 128-byte line
-    // per lane and array) is requested when the current segment starts; a segment longer than
-    // that requests its own later parts kFuHead entries ahead while it is walked (lookahead_in).
-    // The distance is bounded on purpose: fetching a whole long segment early (config 5: rows of
-    // up to 25 000 entries) pushes lines out of the L2 before they are used.
+    // L2 look-ahead.  The head of the NEXT segment (its first kFuHead = 512 entries: lanes 0..15,
+    // one 128-byte line per lane and array) is requested when the current segment starts; a
+    // segment longer than that requests its own later parts kFuDist entries ahead while it is
+    // walked (lookahead_in, 512 entries every 4 steps).  The distance is short on purpose: a line
+    // fetched too early is evicted before it is used and read twice from DRAM (config 5, rows of
+    // up to 25 000 entries: whole segment ahead 5.00 ms, 1024 entries 3.37 ms with 22 % re-reads,
+    // 512 entries 3.10 ms; 256 entries is too little: 3.17 ms, and cfg3 3.37 instead of 3.25).
     auto l2_prefetch = [&](int64_t mb, int64_t me, int ri) {
       const int64_t pb = __shfl_sync(0xffffffffu, mb, ri);
       const int64_t pe = __shfl_sync(0xffffffffu, me, ri);
@@ -860,8 +866,8 @@ __device__ __forceinline__ void fused_stream_body(const FusedArgs& a, uint32_t* 
         asm volatile("prefetch.global.L2 [%0];" ::"l"(a.data + p));
       }
     };
-    auto lookahead_in = [&](int64_t abeg, int span, int st) {  // st % 4 == 0: entries [st 128 + kFuHead, + 512) of this segment
-      const int off = st * 128 + kFuHead + lane * 32;
+    auto lookahead_in = [&](int64_t abeg, int span, int st) {  // st % 4 == 0: entries [st 128 + kFuDist, + 512) of this segment
+      const int off = st * 128 + kFuDist + lane * 32;
       if (lane < 16 && off < span) {
         asm volatile("prefetch.global.L2 [%0];" ::"l"(a.indices + abeg + off));
         asm volatile("prefetch.global.L2 [%0];" ::"l"(a.data + abeg + off));
@@ -955,7 +961,7 @@ __device__ __forceinline__ void fused_stream_body(const FusedArgs& a, uint32_t* 
           for (int st = 0; st < nsteps; ++st) {
             const int4 jc = jn;
             const float4 xc = xn4;
-            if ((st & 3) == 0 && st * 128 + kFuHead < S.head + S.len) lookahead_in(S.abeg, S.head + S.len, st);
+            if ((st & 3) == 0 && st * 128 + kFuDist < S.head + S.len) lookahead_in(S.abeg, S.head + S.len, st);
             if (st + 1 < nsteps) {
               load_step(S, st + 1, jn, xn4);
             } else {                                      // prefetch the next segment's first step
