@@ -87,6 +87,8 @@ uint64_t rsc_kernel_launch_count(void);
  *   "qc_row_budget"    [512]   the same for the QC pass's packed count | total words (1..512)
  *   "grid_ctas"        [0]     CTAs of the streaming kernels, 0 = one per SM
  *   "force_generic"    [0]     1 = always take the generic L2-atomic kernels
+ *   "hvg_single_cta"   [0]     1 = rsc_hvg_select on its one-CTA kernel (default: a cluster of 8 CTAs
+ *                              when n_bins <= 32 and n_genes <= 65 536)
  * Returns RSC_ERR_INVALID_ARG for an unknown key or a value out of range. */
 int rsc_set_option(const char* key, long long value);
 

@@ -118,6 +118,8 @@ int rsc_set_option(const char* key, long long value) {
     g_opt.grid_ctas = (int)value;
   } else if (!strcmp(key, "force_generic")) {
     g_opt.force_generic = value != 0;
+  } else if (!strcmp(key, "hvg_single_cta")) {
+    g_opt.hvg_single_cta = value != 0;
   } else {
     set_error("rsc_set_option: unknown key '%s'", key);
     return RSC_ERR_INVALID_ARG;

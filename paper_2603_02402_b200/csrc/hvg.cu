@@ -507,6 +507,11 @@ hvg_kernel(int G, const double* __restrict__ blk_mm, int n_tblocks, int n_top,
   }
 }
 
+bool hvg_cluster_ok(int32_t G, int32_t n_bins);
+int launch_hvg_cluster(int32_t G, const double* mean, const double* var, int32_t n_top, int32_t n_bins, int flags,
+                       double* m_arr, double* d_arr, double* z_arr, int32_t* b_arr, uint8_t* out_mask,
+                       int32_t* out_indices, int32_t* out_count, cudaStream_t st);
+
 size_t hvg_workspace_bytes(int32_t G, int32_t /*n_bins*/) {
   // m, d, z (double) + bin (int32), each 256-byte aligned
   const size_t tb = ((size_t)G + kHvgTBlock - 1) / kHvgTBlock;
@@ -530,6 +535,9 @@ int launch_hvg(int32_t G, const double* mean, const double* var, int32_t n_top, 
   double* d_arr = out_disp ? out_disp : reinterpret_cast<double*>(w + dsz);
   double* z_arr = out_disp_norm ? out_disp_norm : reinterpret_cast<double*>(w + 2 * dsz);
   int32_t* b_arr = out_bin ? out_bin : reinterpret_cast<int32_t*>(w + 3 * dsz);
+  if (hvg_cluster_ok(G, n_bins) && !g_opt.hvg_single_cta)
+    return launch_hvg_cluster(G, mean, var, n_top, n_bins, flags, m_arr, d_arr, z_arr, b_arr, out_mask, out_indices,
+                              out_count, st);
   const size_t smem = hvg_smem(G, n_bins).total;
   if (smem > 48 * 1024) {
     RSC_CUDA(cudaFuncSetAttribute(hvg_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,

@@ -11,6 +11,7 @@ import torch
 from oracle import oracle_np as O
 from paper_2603_02402_b200 import synth
 import parity_util as U
+from paper_2603_02402_b200 import binding as B  # noqa: E402
 
 pytestmark = pytest.mark.gpu
 
@@ -443,3 +444,34 @@ def test_edge_inputs_misaligned_explicit_zeros_and_empty():
     assert int(q["cell_total_i64"].abs().sum()) == 0 and int(q["gene_n_cells"].abs().sum()) == 0
     out = B.rsc_normalize_log1p_moments(X, s, q["cell_total_i64"], q["gene_n_cells"], 3, 1)
     assert float(out["mean_log"].abs().sum()) == 0 and float(out["var_lin"].abs().sum()) == 0
+
+
+@pytest.mark.parametrize("G,n_top,n_bins", [(7, 3, 20), (1000, 100, 20), (18000, 2000, 20), (36000, 3000, 32), (65536, 5000, 7)])
+def test_hvg_cluster_kernel_equals_single_cta(G, n_top, n_bins):
+    """The cluster kernel (default) and the one-CTA kernel give the same bins, mask, indices and
+    count, and z-scores that differ only by the summation order inside a bin."""
+    rng = np.random.default_rng(G)
+    mean = np.exp(rng.normal(-1.0, 1.5, G)); var = mean * np.exp(rng.normal(0.3, 0.6, G))
+    mean[rng.choice(G, max(1, G // 50), replace=False)] = 0.0
+    var[mean == 0] = 0.0
+    gm, gv = torch.from_numpy(mean).cuda(), torch.from_numpy(var).cuda()
+    a = B.rsc_hvg_select(gm, gv, n_top, n_bins)
+    B.rsc_set_option("hvg_single_cta", 1)
+    try:
+        b = B.rsc_hvg_select(gm, gv, n_top, n_bins)
+    finally:
+        B.rsc_set_option("hvg_single_cta", 0)
+    torch.cuda.synchronize()
+    assert torch.equal(a["bin"], b["bin"]) and torch.equal(a["mean_t"], b["mean_t"])
+    assert torch.equal(torch.nan_to_num(a["disp"], nan=-9.0), torch.nan_to_num(b["disp"], nan=-9.0))
+    za, zb = a["disp_norm"].cpu().numpy(), b["disp_norm"].cpu().numpy()
+    np.testing.assert_allclose(za, zb, rtol=1e-11, atol=1e-12, equal_nan=True)
+    ca, cb = int(a["count"][0]), int(b["count"][0])
+    ma, mb = a["mask"].cpu().numpy().astype(bool), b["mask"].cpu().numpy().astype(bool)
+    d = np.nonzero(ma != mb)[0]                       # only z values tied within rounding at the cutoff may differ
+    if len(d):
+        cut = np.sort(zb[~np.isnan(zb)])[::-1][min(n_top, (~np.isnan(zb)).sum()) - 1]
+        assert np.all(np.abs(zb[d] - cut) <= 1e-9 * max(1.0, abs(cut)))
+    assert np.array_equal(a["indices"].cpu().numpy()[:ca], np.nonzero(ma)[0]) and ca == ma.sum() and cb == mb.sum()
+    o = O.hvg_select(mean, var, n_top, n_bins)
+    U.assert_hvg_matches(a, o, n_top, f"cluster G={G}", strict=False)
