@@ -95,6 +95,7 @@ class ClockSampler(threading.Thread):
         self.index, self.period, self.stop_flag = index, period_s, False
         self.recording = False            # samples are kept only while the timed region runs
         self.sm, self.reasons, self.max_sm, self.ok = [], 0, None, False
+        self.pw, self.mem = [], []
         try:
             import pynvml
             pynvml.nvmlInit()
@@ -114,6 +115,8 @@ class ClockSampler(threading.Thread):
                 if self.recording:
                     self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
                     self.reasons |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                    self.mem.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_MEM))
+                    self.pw.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
             except Exception:
                 pass
             time.sleep(self.period)
@@ -127,8 +130,9 @@ class ClockSampler(threading.Thread):
                  0x100: "display_clock_setting"}
         rs = [v for k, v in names.items() if self.reasons & k and v != "gpu_idle"]
         s = sorted(self.sm)
-        return {"sm_mhz": float(s[len(s) // 2]), "sm_max_mhz": float(self.max_sm), "reasons": rs,
-                "samples": len(s)}
+        return {"sm_mhz": float(s[len(s) // 2]), "sm_mhz_min": float(s[0]), "sm_max_mhz": float(self.max_sm),
+                "reasons": rs, "samples": len(s), "power_w_max": max(self.pw) if self.pw else None,
+                "mem_mhz_min": min(self.mem) if self.mem else None}
 
 
 # ------------------------------------------------------------------------------ CPU oracle legs
