@@ -475,3 +475,38 @@ def test_hvg_cluster_kernel_equals_single_cta(G, n_top, n_bins):
     assert np.array_equal(a["indices"].cpu().numpy()[:ca], np.nonzero(ma)[0]) and ca == ma.sum() and cb == mb.sum()
     o = O.hvg_select(mean, var, n_top, n_bins)
     U.assert_hvg_matches(a, o, n_top, f"cluster G={G}", strict=False)
+
+
+@pytest.mark.parametrize("case", ["one_bin", "all_equal_means", "infinite_z", "all_nan", "n_top_huge", "max_bins"])
+def test_hvg_cluster_kernel_degenerate_cases(case):
+    """Degenerate inputs through the cluster kernel against the oracle (and the one-CTA kernel)."""
+    rng = np.random.default_rng(5)
+    G, n_top, n_bins = 3000, 300, 20
+    mean = np.exp(rng.normal(-1.0, 1.5, G)); var = mean * np.exp(rng.normal(0.3, 0.6, G))
+    if case == "one_bin":
+        n_bins = 1
+    elif case == "all_equal_means":
+        mean[:] = 0.7
+    elif case == "infinite_z":                       # a bin whose members share one dispersion: sd = 0 -> z = 0/0 or x/0
+        mean[:40] = np.linspace(5.0, 5.001, 40); var[:40] = 2.0 * mean[:40]
+        mean[40] = 5.0005; var[40] = 9.0 * mean[40]
+        n_bins = 32
+    elif case == "all_nan":
+        var[:] = 0.0                                 # d = 0 -> NaN after the Seurat transform: nothing is selectable
+    elif case == "n_top_huge":
+        n_top = 10 * G
+    elif case == "max_bins":
+        n_bins = 32
+    gm, gv = torch.from_numpy(mean).cuda(), torch.from_numpy(var).cuda()
+    a = B.rsc_hvg_select(gm, gv, n_top, n_bins)
+    B.rsc_set_option("hvg_single_cta", 1)
+    try:
+        b = B.rsc_hvg_select(gm, gv, n_top, n_bins)
+    finally:
+        B.rsc_set_option("hvg_single_cta", 0)
+    torch.cuda.synchronize()
+    o = O.hvg_select(mean, var, n_top, n_bins)
+    U.assert_hvg_matches(a, o, n_top, f"cluster {case}", strict=False)
+    U.assert_hvg_matches(b, o, n_top, f"one CTA {case}", strict=False)
+    assert torch.equal(a["bin"], b["bin"]) and int(a["count"][0]) == int(b["count"][0])
+    assert torch.equal(a["mask"], b["mask"])
