@@ -463,6 +463,16 @@ def main():
                          "peak_source": peak_src + " bf16_tflops (burst); fp16 = bf16 rate (guide's nominal ratio 1)",
                          "flops": "3 n p^2: hi*hi + hi*lo + lo*hi on the upper triangle; tile padding not counted"},
             "note": "whole rsc_gram_cov call: exact mean (moments pass), pack to fp16 hi/lo planes, MMA, finalize"}
+        # log-scale moments of the HVG columns only: what `scale` needs when the chain ran with the
+        # linear-scale set alone (the scanpy order: HVG from x', scale on the subset) -- the cheap
+        # alternative to which_moments = 3
+        ms, _mm = timed(torch, lambda: binding.rsc_gene_moments(Y, 0, 1), reps=3, warm=2)
+        nxt["gene_moments (HVG columns, log scale)"] = {
+            "ms": ms, "GBps": 8.0 * Y.nnz / (ms / 1e3) / 1e9,
+            "note": "with variants.which_moments=2 this replaces the two-set fused pass: chain(2) + subset + this"}
+        if variants is not None and "which_moments=2" in variants:
+            nxt["gene_moments (HVG columns, log scale)"]["two_set_workflow_ms"] = \
+                variants["which_moments=2"]["chain_ms"] + ms
         # the projection of L95 on 50 loadings (orthonormal random V: the eigensolver is a library call)
         Vq = torch.linalg.qr(torch.randn(g2, 50, dtype=torch.float64, device=dev))[0].contiguous()
         mu64 = out_h["mean_log"][sel].contiguous()
