@@ -505,7 +505,8 @@ def main():
             ms = statistics.median(ts)
             r = {"value": nnz / (ms / 1e3), "unit": UNIT, "ms_per_step": ms,
                  "h2d_bytes_per_step": hp.h2d_bytes, "d2h_bytes_per_step": hp.d2h_bytes,
-                 "note": "rsc_preprocess_host: pinned host CSR in, all QC/moment/HVG arrays out; " +
+                 "note": "rsc_preprocess_host: pinned host CSR in (row chunks: H2D of chunk k+1 and D2H of chunk k-1 "
+                         "beside the kernels of chunk k), all QC/moment/HVG arrays out; " +
                          ("the log-normalised x'' copied back to the host as well" if roundtrip else
                           "x'' stays on the device")}
             if roundtrip:

@@ -87,6 +87,8 @@ uint64_t rsc_kernel_launch_count(void);
  *   "qc_row_budget"    [512]   the same for the QC pass's packed count | total words (1..512)
  *   "grid_ctas"        [0]     CTAs of the streaming kernels, 0 = one per SM
  *   "force_generic"    [0]     1 = always take the generic L2-atomic kernels
+ *   "host_chunk_nnz"   [150e6] rsc_preprocess_host: stored entries per pipelined row chunk (at most 16
+ *                              chunks; 0 = one chunk: copy in, compute, copy out one after the other)
  *   "hvg_single_cta"   [0]     1 = rsc_hvg_select on its one-CTA kernel (default: a cluster of 8 CTAs
  *                              when n_bins <= 32 and n_genes <= 65 536)
  * Returns RSC_ERR_INVALID_ARG for an unknown key or a value out of range. */
@@ -406,9 +408,13 @@ int rsc_preprocess(rsc_csr* X, const uint8_t* gene_flags, const rsc_params* prm,
  * HOST pointers (pinned memory recommended), `host_out` HOST output pointers (any may
  * be NULL); `host_data_out` optionally receives the log-normalised values.  The call
  * stages everything through the caller's device workspace `dev_ws` (size from
- * rsc_preprocess_host_workspace_bytes), enqueues H2D copies, the chain and D2H copies
- * on `stream`, and returns without synchronising; the caller synchronises the stream
- * before reading the host outputs.
+ * rsc_preprocess_host_workspace_bytes) and returns without synchronising; the caller
+ * synchronises `stream` before reading the host outputs.  The matrix travels in row chunks: the
+ * kernels of chunk k run on `stream` while chunk k + 1 is copied in and the x'' of chunk k - 1 is
+ * copied out on two copy streams the library keeps per host thread and device (they start after
+ * the work already queued on `stream`, and `stream` waits for them before the call's last
+ * copies); the per-gene results of the chunks are added in chunk order.  Pinned host memory is
+ * needed for the copies to overlap.
  * ------------------------------------------------------------------------------- */
 size_t rsc_preprocess_host_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz, int32_t n_bins);
 int rsc_preprocess_host(const rsc_csr* host_X, const uint8_t* host_gene_flags,

@@ -101,8 +101,12 @@ struct HostWs {
   int64_t* indptr; int32_t* indices; float* data; uint8_t* flags;
   rsc_outputs o;
   void* chain_ws; size_t chain_bytes;
+  // per-gene partial results of the row chunks (kHostMaxChunks each)
+  int32_t* part_n_cells; int64_t* part_total; double* part_sums;   // [C][G], [C][G], [C][4 G]
+  double* sums;                                                     // [4 G] added over the chunks
   size_t total;
 };
+constexpr int kHostMaxChunks = 16;
 
 static HostWs carve_host(void* ws, int64_t n, int32_t G, int64_t nnz, int32_t n_bins) {
   Carver c(ws);
@@ -131,8 +135,52 @@ static HostWs carve_host(void* ws, int64_t n, int32_t G, int64_t nnz, int32_t n_
   h.o.hvg_count = c.take<int32_t>(1);
   h.chain_bytes = carve_chain(nullptr, n, G, nnz, n_bins).total;
   h.chain_ws = c.take_bytes(h.chain_bytes);
+  h.part_n_cells = c.take<int32_t>((size_t)kHostMaxChunks * (size_t)G);
+  h.part_total = c.take<int64_t>((size_t)kHostMaxChunks * (size_t)G);
+  h.part_sums = c.take<double>((size_t)kHostMaxChunks * 4 * (size_t)G);
+  h.sums = c.take<double>(4 * (size_t)G);
   h.total = c.off;
   return h;
+}
+
+// per-gene results of the row chunks added up (chunk order: a fixed summation order)
+__global__ void __launch_bounds__(256)
+host_chunk_reduce_kernel(int32_t G, int C, const int32_t* __restrict__ part_n_cells,
+                         const int64_t* __restrict__ part_total, const double* __restrict__ part_sums,
+                         int32_t* __restrict__ gene_n_cells, int64_t* __restrict__ gene_total,
+                         double* __restrict__ sums) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= G) return;
+  int32_t nc = 0;
+  int64_t tt = 0;
+  double s[4] = {0.0, 0.0, 0.0, 0.0};
+  for (int c = 0; c < C; ++c) {
+    nc += part_n_cells[(size_t)c * G + g];
+    tt += part_total[(size_t)c * G + g];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) s[k] += part_sums[((size_t)c * 4 + k) * G + g];
+  }
+  if (gene_n_cells) gene_n_cells[g] = nc;
+  if (gene_total) gene_total[g] = tt;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) sums[(size_t)k * G + g] = s[k];
+}
+
+// copy streams of the host entry point (one pair per host thread and device, created on first
+// use and kept): the H2D copy of chunk k + 1 and the D2H copy of chunk k - 1 run beside the
+// kernels of chunk k, which stay on the caller's stream
+struct CopyStreams { int dev = -1; cudaStream_t in = nullptr, out = nullptr; };
+static thread_local CopyStreams g_copy;
+static int copy_streams(cudaStream_t* in, cudaStream_t* out) {
+  int dev = -1;
+  RSC_CUDA(cudaGetDevice(&dev));
+  if (g_copy.dev != dev) {
+    RSC_CUDA(cudaStreamCreateWithFlags(&g_copy.in, cudaStreamNonBlocking));
+    RSC_CUDA(cudaStreamCreateWithFlags(&g_copy.out, cudaStreamNonBlocking));
+    g_copy.dev = dev;
+  }
+  *in = g_copy.in; *out = g_copy.out;
+  return RSC_OK;
 }
 
 template <typename T>
@@ -196,18 +244,112 @@ int rsc_preprocess_host(const rsc_csr* hX, const uint8_t* host_gene_flags, const
   }
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   RSC_CUDA(cudaMemcpyAsync(h.indptr, hX->indptr, sizeof(int64_t) * (size_t)(n + 1), cudaMemcpyHostToDevice, st));
-  if (nnz) {
-    RSC_CUDA(cudaMemcpyAsync(h.indices, hX->indices, sizeof(int32_t) * (size_t)nnz, cudaMemcpyHostToDevice, st));
-    RSC_CUDA(cudaMemcpyAsync(h.data, hX->data, sizeof(float) * (size_t)nnz, cudaMemcpyHostToDevice, st));
-  }
   const uint8_t* dflags = nullptr;
   if (host_gene_flags) {
     RSC_CUDA(cudaMemcpyAsync(h.flags, host_gene_flags, (size_t)G, cudaMemcpyHostToDevice, st));
     dflags = h.flags;
   }
-  rsc_csr dX = *hX;
-  dX.indptr = h.indptr; dX.indices = h.indices; dX.data = h.data;
-  if ((rc = run_chain(&dX, dflags, prm, &h.o, h.chain_ws, st))) return rc;
+  // Row chunks of ~host_chunk_nnz stored entries (option; 150 M = 1.2 GB of H2D by default) (cut on the host from the host indptr).  The two
+  // streaming passes need nothing beyond a chunk's own rows (the per-cell totals are row-local),
+  // so chunk k is computed -- on the caller's stream -- while chunk k + 1 is copied in and the
+  // x'' of chunk k - 1 is copied out on the two copy streams (PCIe is full duplex); the per-gene
+  // results of the chunks are added up at the end, then moments, then HVG.
+  const int64_t chunk_nnz = g_opt.host_chunk_nnz.load() > 0 ? (int64_t)g_opt.host_chunk_nnz.load() : nnz + 1;
+  int64_t Cl = (nnz + chunk_nnz - 1) / chunk_nnz;
+  int C = (int)(Cl > kHostMaxChunks ? kHostMaxChunks : Cl);
+  C = C < 1 ? 1 : (C > kHostMaxChunks ? kHostMaxChunks : C);
+  if (n < 4 * (int64_t)C) C = 1;
+  int64_t rb[kHostMaxChunks + 1];
+  rb[0] = 0;
+  for (int c = 1; c < C; ++c) {                            // first row whose offset reaches c nnz / C
+    const int64_t target = (int64_t)((double)nnz * c / C);
+    int64_t lo = rb[c - 1], hi = n;
+    while (lo < hi) {
+      const int64_t mid = (lo + hi) >> 1;
+      if (hX->indptr[mid] < target) lo = mid + 1; else hi = mid;
+    }
+    rb[c] = lo;
+  }
+  rb[C] = n;
+  cudaStream_t s_in = st, s_out = st;
+  cudaEvent_t ev_fork = nullptr, ev_in[kHostMaxChunks] = {}, ev_cmp[kHostMaxChunks] = {}, ev_out = nullptr;
+  const bool piped = C > 1;
+  if (piped) {
+    if ((rc = copy_streams(&s_in, &s_out))) return rc;
+    RSC_CUDA(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
+    RSC_CUDA(cudaEventCreateWithFlags(&ev_out, cudaEventDisableTiming));
+    RSC_CUDA(cudaEventRecord(ev_fork, st));                // the copy streams start after the caller's earlier work
+    RSC_CUDA(cudaStreamWaitEvent(s_in, ev_fork, 0));
+    RSC_CUDA(cudaStreamWaitEvent(s_out, ev_fork, 0));
+  }
+  ChainWs w = carve_chain(h.chain_ws, n, G, nnz, prm->n_bins);
+  const size_t K1 = (size_t)split_blocks(G) + 1;
+  int32_t need[32];
+  int32_t n_need = fused_split_blocks(G, prm->which_moments, need, 32);
+  if (n_need > 32) n_need = 0;
+  const bool sorted = (hX->flags & RSC_CSR_SORTED) != 0;
+  for (int c = 0; c < C; ++c) {
+    const int64_t r0 = rb[c], r1 = rb[c + 1];
+    const int64_t p0 = hX->indptr[r0], p1 = hX->indptr[r1];
+    if (p1 > p0) {
+      RSC_CUDA(cudaMemcpyAsync(h.indices + p0, hX->indices + p0, sizeof(int32_t) * (size_t)(p1 - p0), cudaMemcpyHostToDevice, s_in));
+      RSC_CUDA(cudaMemcpyAsync(h.data + p0, hX->data + p0, sizeof(float) * (size_t)(p1 - p0), cudaMemcpyHostToDevice, s_in));
+    }
+    if (piped) {
+      RSC_CUDA(cudaEventCreateWithFlags(&ev_in[c], cudaEventDisableTiming));
+      RSC_CUDA(cudaEventRecord(ev_in[c], s_in));
+      RSC_CUDA(cudaStreamWaitEvent(st, ev_in[c], 0));
+    }
+    // the chunk as a CSR view: absolute offsets, so indices / data keep their base pointers
+    rsc_csr Xc = *hX;
+    Xc.n_rows = r1 - r0; Xc.indptr = h.indptr + r0; Xc.indices = h.indices; Xc.data = h.data;
+    uint32_t* splits = sorted ? w.splits + (size_t)r0 * K1 : nullptr;
+    int32_t* pn = h.part_n_cells + (size_t)c * G;
+    int64_t* pt = h.part_total + (size_t)c * G;
+    double* ps = h.part_sums + (size_t)c * 4 * G;
+    RSC_CUDA(cudaMemsetAsync(ps, 0, sizeof(double) * 4 * (size_t)G, st));
+    rc = launch_qc(Xc, dflags, h.o.cell_total_i64 + r0, h.o.cell_total_f32 + r0, h.o.cell_n_genes + r0,
+                   h.o.cell_flag_total_i64 + r0, h.o.cell_flag_pct + r0, pn, pt, splits, need, n_need,
+                   w.qc_ws, w.qc_bytes, st);
+    if (rc) return rc;
+    rc = launch_fused(Xc, prm->target_sum, h.o.cell_total_i64 + r0, pn, splits, prm->which_moments, prm->ddof,
+                      w.mean_log, w.var_log, w.mean_lin, w.var_lin, ps, w.fused_ws, w.fused_bytes, st);
+    if (rc) return rc;
+    if (host_data_out && p1 > p0) {
+      if (piped) {
+        RSC_CUDA(cudaEventCreateWithFlags(&ev_cmp[c], cudaEventDisableTiming));
+        RSC_CUDA(cudaEventRecord(ev_cmp[c], st));
+        RSC_CUDA(cudaStreamWaitEvent(s_out, ev_cmp[c], 0));
+      }
+      RSC_CUDA(cudaMemcpyAsync(host_data_out + p0, h.data + p0, sizeof(float) * (size_t)(p1 - p0), cudaMemcpyDeviceToHost, s_out));
+    }
+  }
+  host_chunk_reduce_kernel<<<(G + 255) / 256, 256, 0, st>>>(G, C, h.part_n_cells, h.part_total, h.part_sums,
+                                                           h.o.gene_n_cells, h.o.gene_total_i64, h.sums);
+  RSC_LAUNCH_CHECK("host_chunk_reduce_kernel");
+  const size_t sG = (size_t)G;
+  if (prm->which_moments & RSC_MOMENTS_LOG)
+    if ((rc = finalize_moments(G, n, prm->ddof, h.sums, h.sums + sG, h.o.mean_log, h.o.var_log, st))) return rc;
+  if (prm->which_moments & RSC_MOMENTS_LIN)
+    if ((rc = finalize_moments(G, n, prm->ddof, h.sums + 2 * sG, h.sums + 3 * sG, h.o.mean_lin, h.o.var_lin, st))) return rc;
+  {
+    const double* hm = prm->hvg_on_linear ? h.o.mean_lin : h.o.mean_log;
+    const double* hv = prm->hvg_on_linear ? h.o.var_lin : h.o.var_log;
+    rc = launch_hvg(G, hm, hv, prm->n_top, prm->n_bins, prm->hvg_flags, h.o.hvg_mean_t, h.o.hvg_disp,
+                    h.o.hvg_disp_norm, h.o.hvg_bin, h.o.hvg_mask, h.o.hvg_indices, h.o.hvg_count, w.hvg_ws,
+                    w.hvg_bytes, st);
+    if (rc) return rc;
+  }
+  if (piped) {                                             // join: the caller's stream also waits for the copies out
+    RSC_CUDA(cudaEventRecord(ev_out, s_out));
+    RSC_CUDA(cudaStreamWaitEvent(st, ev_out, 0));
+    for (int c = 0; c < C; ++c) {
+      if (ev_in[c]) cudaEventDestroy(ev_in[c]);            // released by the runtime once they have completed
+      if (ev_cmp[c]) cudaEventDestroy(ev_cmp[c]);
+    }
+    cudaEventDestroy(ev_fork);
+    cudaEventDestroy(ev_out);
+  }
   const size_t sn = (size_t)n, sg = (size_t)G;
   if ((rc = d2h(ho->cell_total_i64, h.o.cell_total_i64, sn, st))) return rc;
   if ((rc = d2h(ho->cell_total_f32, h.o.cell_total_f32, sn, st))) return rc;
@@ -231,9 +373,6 @@ int rsc_preprocess_host(const rsc_csr* hX, const uint8_t* host_gene_flags, const
   if ((rc = d2h(ho->hvg_mask, h.o.hvg_mask, sg, st))) return rc;
   if ((rc = d2h(ho->hvg_indices, h.o.hvg_indices, sg, st))) return rc;
   if ((rc = d2h(ho->hvg_count, h.o.hvg_count, 1, st))) return rc;
-  if (host_data_out && nnz) {
-    RSC_CUDA(cudaMemcpyAsync(host_data_out, h.data, sizeof(float) * (size_t)nnz, cudaMemcpyDeviceToHost, st));
-  }
   return RSC_OK;
 }
 

@@ -46,6 +46,7 @@ struct Options {                  // process-wide, set through rsc_set_option; a
   std::atomic<int> qc_row_budget{512};        // rows a QC CTA takes between two checks of its table (<= 512)
   std::atomic<int> grid_ctas{0};              // CTAs of the streaming kernels; 0 = one per SM
   std::atomic<int> force_generic{0};          // 1: always use the generic L2-atomic kernels
+  std::atomic<long long> host_chunk_nnz{150000000};   // rsc_preprocess_host: stored entries per pipelined row chunk
   std::atomic<int> hvg_single_cta{0};         // 1: rsc_hvg_select on the one-CTA kernel (not the cluster kernel)
 };
 extern Options g_opt;

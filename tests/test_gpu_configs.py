@@ -251,7 +251,19 @@ def test_config4_int64_nnz_sampled():
     assert nnz > 2**31
 
 
-def test_host_entry_point_matches_device_chain():
+@pytest.mark.parametrize("chunk_nnz", [0, 150_000_000, 200_000, 37_000])
+def test_host_entry_point_matches_device_chain(chunk_nnz):
+    """rsc_preprocess_host against the device chain: one chunk (0), the default, 9 and 16 pipelined
+    row chunks (H2D of chunk k + 1 and D2H of chunk k - 1 beside the kernels of chunk k)."""
+    from paper_2603_02402_b200 import Csr, HostPreprocessor, binding
+    binding.rsc_set_option("host_chunk_nnz", chunk_nnz)
+    try:
+        _host_entry_point_check()
+    finally:
+        binding.rsc_set_option("host_chunk_nnz", 150_000_000)
+
+
+def _host_entry_point_check():
     from paper_2603_02402_b200 import Csr, HostPreprocessor
     cfg = synth.CONFIGS[1]
     indptr, indices, data = synth.make_csr(cfg, "cuda", n_cells=1200)
