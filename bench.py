@@ -404,6 +404,20 @@ def main():
                                                "chain_ms": statistics.median(t["step"]),
                                                "chain_nnz_per_s": nnz / (statistics.median(t["step"]) / 1e3)}
             del vp
+        # the one-pass chain (csrc/single.cu, option "single_pass"): QC folded into the fused pass by
+        # pairs of CTAs; 12 B / nnz of DRAM traffic, but more instructions than the two passes together
+        if args.which_moments == 1 and cfg.n_genes <= 32768:
+            sp = Preprocessor(X.n_rows, X.n_cols, nnz, cfg.target_sum, cfg.n_top, cfg.n_bins, 1, 1, False, device=dev)
+            binding.rsc_set_option("single_pass", 1)
+            try:
+                ms_sp, _ = timed(torch, lambda: sp.run(X, flags), reps=5, warm=2,
+                                 before=lambda: data.copy_(pristine))
+            finally:
+                binding.rsc_set_option("single_pass", 0)
+            variants["single_pass"] = {"chain_ms": ms_sp, "chain_nnz_per_s": nnz / (ms_sp / 1e3),
+                                       "dram_bytes_per_nnz": 12.0,
+                                       "note": "rsc_preprocess with option single_pass=1 (not the default)"}
+            del sp
 
     # ---- the unfused entry points, 8 B / nnz each
     unfused = None

@@ -89,6 +89,12 @@ uint64_t rsc_kernel_launch_count(void);
  *   "force_generic"    [0]     1 = always take the generic L2-atomic kernels
  *   "host_chunk_nnz"   [150e6] rsc_preprocess_host: stored entries per pipelined row chunk (at most 16
  *                              chunks; 0 = one chunk: copy in, compute, copy out one after the other)
+ *   "single_pass"      [0]     1 = rsc_preprocess runs QC + normalise + log1p + log-scale moments as ONE pass
+ *                              over the matrix (pairs of CTAs exchanging the rows' partial totals through
+ *                              distributed shared memory: 12 B / nnz of DRAM traffic instead of 20) when it
+ *                              can: sorted rows, 16-byte aligned arrays, 512 <= n_cols <= 32 768,
+ *                              n_rows < 2^24, which_moments == RSC_MOMENTS_LOG.  Same results (integers and
+ *                              x'' bit for bit); slower than the default two passes on B200
  *   "hvg_single_cta"   [0]     1 = rsc_hvg_select on its one-CTA kernel (default: a cluster of 8 CTAs
  *                              when n_bins <= 32 and n_genes <= 65 536)
  * Returns RSC_ERR_INVALID_ARG for an unknown key or a value out of range. */

@@ -121,6 +121,8 @@ int rsc_set_option(const char* key, long long value) {
   } else if (!strcmp(key, "host_chunk_nnz")) {
     RSC_CHECK_ARG(value >= 0, "rsc_set_option: host_chunk_nnz must be >= 0");
     g_opt.host_chunk_nnz = value;
+  } else if (!strcmp(key, "single_pass")) {
+    g_opt.single_pass = value != 0;
   } else if (!strcmp(key, "hvg_single_cta")) {
     g_opt.hvg_single_cta = value != 0;
   } else {

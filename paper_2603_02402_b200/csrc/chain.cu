@@ -78,6 +78,17 @@ static int run_chain(rsc_csr* X, const uint8_t* gene_flags, const rsc_params* pr
   double* mean_lin = out->mean_lin ? out->mean_lin : w.mean_lin;
   double* var_lin = out->var_lin ? out->var_lin : w.var_lin;
 
+  if (single_pass_ok(*X, prm->which_moments) && !prm->hvg_on_linear &&
+      single_workspace_bytes(X->n_rows, X->n_cols, X->nnz) <= w.fused_bytes) {
+    // one pass over the matrix: QC + normalise + log1p + log-scale moments (single.cu)
+    int rc1 = launch_single_pass(*X, gene_flags, prm->target_sum, prm->ddof, cell_total, out->cell_total_f32,
+                                 out->cell_n_genes, out->cell_flag_total_i64, out->cell_flag_pct, gene_n_cells,
+                                 out->gene_total_i64, mean_log, var_log, w.fused_ws, st);
+    if (rc1) return rc1;
+    return launch_hvg(X->n_cols, mean_log, var_log, prm->n_top, prm->n_bins, prm->hvg_flags, out->hvg_mean_t,
+                      out->hvg_disp, out->hvg_disp_norm, out->hvg_bin, out->hvg_mask, out->hvg_indices,
+                      out->hvg_count, w.hvg_ws, w.hvg_bytes, st);
+  }
   uint32_t* splits = (X->flags & RSC_CSR_SORTED) ? w.splits : nullptr;
   // only the split entries the fused pass will read (its group edges) are produced
   int32_t need[32];

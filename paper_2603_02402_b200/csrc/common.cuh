@@ -47,6 +47,7 @@ struct Options {                  // process-wide, set through rsc_set_option; a
   std::atomic<int> grid_ctas{0};              // CTAs of the streaming kernels; 0 = one per SM
   std::atomic<int> force_generic{0};          // 1: always use the generic L2-atomic kernels
   std::atomic<long long> host_chunk_nnz{150000000};   // rsc_preprocess_host: stored entries per pipelined row chunk
+  std::atomic<int> single_pass{0};            // 1: rsc_preprocess takes the one-pass cluster kernel (single.cu) when it can
   std::atomic<int> hvg_single_cta{0};         // 1: rsc_hvg_select on the one-CTA kernel (not the cluster kernel)
 };
 extern Options g_opt;
@@ -133,6 +134,12 @@ size_t pca_workspace_bytes(int32_t n_cols, int32_t n_comps);
 bool pca_supported(int32_t n_comps);
 int launch_pca_transform(const rsc_csr& X, const double* V, const double* mean, int32_t k, float* out, void* ws,
                          cudaStream_t st);
+bool single_pass_ok(const rsc_csr& X, int which);
+size_t single_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
+int launch_single_pass(const rsc_csr& X, const uint8_t* gene_flags, float target_sum, int ddof,
+                       int64_t* cell_total_i64, float* cell_total_f32, int32_t* cell_n_genes,
+                       int64_t* cell_flag_total_i64, float* cell_flag_pct, int32_t* gene_n_cells,
+                       int64_t* gene_total_i64, double* mean_log, double* var_log, void* ws, cudaStream_t st);
 size_t gram_workspace_bytes(int64_t n_rows, int32_t n_cols, int64_t nnz);
 bool gram_supported(int32_t n_cols);
 int launch_gram_cov(const rsc_csr& X, double* out_mean, double* out_gram, double* out_cov, void* ws,
