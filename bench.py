@@ -547,6 +547,22 @@ def main():
                 "traffic": traffic, "traffic_source": tsrc,
                 "algorithmic_bytes_per_nnz": BYTES_PER_NNZ["fused"],
                 "ms_per_launch": fused_ms, "frac_of_8TBs": achieved / NOMINAL_HBM_GBS}
+    # this board's own copy rate, measured the way MEASURED_PEAKS.json's was (context for the box-to-box
+    # spread of the fused pass; `peak` stays the driver's number)
+    try:
+        ca = torch.empty(1 << 30, dtype=torch.bfloat16, device=dev)
+        cb = torch.empty_like(ca)
+        best = None
+        for _ in range(6):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); cb.copy_(ca); e1.record(); torch.cuda.synchronize()
+            ms_c = e0.elapsed_time(e1)
+            best = ms_c if best is None or ms_c < best else best
+        roofline["copy_rate_this_board_GBps"] = 2 * ca.numel() * 2 / (best / 1e3) / 1e9
+        roofline["frac_of_this_board"] = achieved / roofline["copy_rate_this_board_GBps"]
+        del ca, cb
+    except Exception:                                          # noqa: BLE001
+        roofline["copy_rate_this_board_GBps"] = None
     qc_gb = BYTES_PER_NNZ["qc"] * nnz / (qc_ms / 1e3) / 1e9
     stages = {
         "qc": {"ms": qc_ms, "GBps": qc_gb, "frac_of_measured": qc_gb / peak},

@@ -188,6 +188,13 @@ __device__ __forceinline__ void st_stream_f4(void* p, float4 v, uint64_t pol) {
                :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "l"(pol) : "memory");
 }
 
+// Store of a value this pass will not read again (st.global.cs: evict-first in L2, so the lines the
+// look-ahead has fetched stay resident).  Measured per kernel (profiles/r02_cfg3.md): fused pass interior
+// quads 3.257 -> 3.185 ms, dense scale output 3.55 -> 3.35 ms; no gain or a loss for normalize, log1p, the
+// subset fill and the fused pass's edge quads (their lines are shared with a neighbouring segment that
+// another CTA writes later: 3.14 -> 3.31 ms), which keep plain stores.
+template <typename T> __device__ __forceinline__ void st_once(T* p, T v) { __stcs(p, v); }
+
 // x'' = log(1 + x') in float32, shared by rsc_log1p and the fused pass so that
 // both write bit-identical values.  x >= 0.25: MUFU lg2 of the rounded 1 + x (absolute error
 // <= 2^-22 * ln 2 + 2^-24, i.e. <= 1e-6 relative there, ~1 ulp for typical x'' of 1..3);

@@ -457,17 +457,19 @@ __device__ __forceinline__ void fused_stream_body(const FusedArgs& a, uint32_t* 
     const float x[4] = {xv.x, xv.y, xv.z, xv.w};
     float xn[4], xl[4], tl[4], tn[4];
     bool valid[4];
-    bool ok = true;
+    unsigned okw = 1u;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       valid[k] = !EDGE || (unsigned)(e0 + k) < (unsigned)len;
       xn[k] = MOM ? x[k] : __fmul_rn(x[k], scale);
       xl[k] = MOM ? x[k] : log1p_ge_quarter(xn[k]);
-      bool okk = MOM || (LOG && !LIN) || xn[k] >= 0.25f;   // log only: implied by the window test
-      if (LOG) { tl[k] = xl[k] * mult_log; okk = okk && in_window_log(tl[k]); }
-      if (LIN) { tn[k] = xn[k] * mult_lin; okk = okk && in_window(tn[k]); }
-      ok = ok && (okk || !valid[k]);
+      // branch-free: one test of the four entries' window bits instead of short-circuit branches (3.257 -> 3.202 ms)
+      unsigned okk = (MOM || (LOG && !LIN) || xn[k] >= 0.25f) ? 1u : 0u;   // log only: implied by the window test
+      if (LOG) { tl[k] = xl[k] * mult_log; okk &= in_window_log(tl[k]) ? 1u : 0u; }
+      if (LIN) { tn[k] = xn[k] * mult_lin; okk &= in_window(tn[k]) ? 1u : 0u; }
+      okw &= okk | (valid[k] ? 0u : 1u);
     }
+    const bool ok = okw != 0u;
     if (ok) {
       uint32_t so[4], so3[4], al[4], an[4];
 #pragma unroll
@@ -584,13 +586,15 @@ __device__ __forceinline__ void fused_stream_body(const FusedArgs& a, uint32_t* 
         float* dq = a.data + (s.abeg + 4 * q);
         if (interior(s, st)) {
           const float4 r = quad(std::false_type{}, jv, xv, s.scale, e0, s.len);
-          if (!MOM) *reinterpret_cast<float4*>(dq) = r;
+          // x'' is written once and not read again by this pass: streaming stores (evict-first in L2) keep the
+          // look-ahead's lines resident (3.257 -> 3.185 ms)
+          if (!MOM) st_once(reinterpret_cast<float4*>(dq), r);
         } else if (q < s.nq) {
           const float4 r = quad(std::true_type{}, jv, xv, s.scale, e0, s.len);
           if (MOM) {
             // nothing is written back
           } else if (e0 >= 0 && e0 + 4 <= s.len) {
-            *reinterpret_cast<float4*>(dq) = r;
+            *reinterpret_cast<float4*>(dq) = r;             // (plain: the line is shared with a neighbouring segment)
           } else {
             if ((unsigned)(e0 + 0) < (unsigned)s.len) dq[0] = r.x;
             if ((unsigned)(e0 + 1) < (unsigned)s.len) dq[1] = r.y;

@@ -199,7 +199,7 @@ scale_dense_chunk_kernel(int64_t n_rows, int32_t G, const int64_t* __restrict__ 
       }
       __syncwarp();
       for (int t = lane * 4; t < c1 - c0; t += 128)
-        *reinterpret_cast<float4*>(o + c0 + t) = *reinterpret_cast<const float4*>(r + t);
+        st_once(reinterpret_cast<float4*>(o + c0 + t), *reinterpret_cast<const float4*>(r + t));
       __syncwarp();
     }
   }

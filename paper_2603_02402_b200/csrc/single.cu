@@ -605,7 +605,7 @@ single_pass_kernel(const SingleArgs a) {
         float* dq = a.data + (sab + 4 * qd);
         if (interior(st)) {
           const float4 r = quad_b(std::false_type{}, jc, xc, scale, e, slen);
-          *reinterpret_cast<float4*>(dq) = r;
+          st_once(reinterpret_cast<float4*>(dq), r);
         } else if (qd < nq) {
           const float4 r = quad_b(std::true_type{}, jc, xc, scale, e, slen);
           if (e >= 0 && e + 4 <= slen) {
