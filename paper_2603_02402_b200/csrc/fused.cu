@@ -560,46 +560,56 @@ __device__ __forceinline__ void fused_stream_body(const FusedArgs& a, uint32_t* 
       auto interior = [&](const Seg& s, int st) -> bool {
         return (st > 0 || s.head == 0) && (st * 128 + 128 <= s.head + s.len);
       };
-      auto load_step = [&](const Seg& s, int st, int4& jv, float4& xv) {
-        const int q = st * 32 + lane;
-        const int64_t off = s.abeg + 4 * q;
+      // dp: this lane's quad of step st in the data array (a running pointer: one add per step instead of
+      // rebuilding the 64-bit address from the step number: 3.139 -> 3.083 ms); the index array lies a fixed
+      // distance away
+      const ptrdiff_t idelta = reinterpret_cast<const char*>(a.indices) - reinterpret_cast<const char*>(a.data);
+      auto idx_of = [&](const float* dp) -> const int32_t* {
+        return reinterpret_cast<const int32_t*>(reinterpret_cast<const char*>(dp) + idelta);
+      };
+      auto load_step = [&](const Seg& s, int st, const float* dp, int4& jv, float4& xv) {
+        const int32_t* ip = idx_of(dp);
         if (interior(s, st)) {
-          jv = __ldg(reinterpret_cast<const int4*>(a.indices + off));
-          xv = *reinterpret_cast<const float4*>(a.data + off);
-        } else if (q < s.nq) {
-          if (off + 4 <= a.nnz) {
-            jv = __ldg(reinterpret_cast<const int4*>(a.indices + off));
-            xv = *reinterpret_cast<const float4*>(a.data + off);
-          } else {                                        // the last quad of the whole matrix
-            const int e0 = q * 4 - s.head;
-            jv = make_int4(0, 0, 0, 0);
-            xv = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (e0 + 0 < s.len) { jv.x = __ldg(a.indices + off + 0); xv.x = a.data[off + 0]; }
-            if (e0 + 1 < s.len) { jv.y = __ldg(a.indices + off + 1); xv.y = a.data[off + 1]; }
-            if (e0 + 2 < s.len) { jv.z = __ldg(a.indices + off + 2); xv.z = a.data[off + 2]; }
+          jv = __ldg(reinterpret_cast<const int4*>(ip));
+          xv = *reinterpret_cast<const float4*>(dp);
+        } else {
+          const int q = st * 32 + lane;
+          if (q < s.nq) {
+            if ((dp - a.data) + 4 <= a.nnz) {
+              jv = __ldg(reinterpret_cast<const int4*>(ip));
+              xv = *reinterpret_cast<const float4*>(dp);
+            } else {                                      // the last quad of the whole matrix
+              const int e0 = q * 4 - s.head;
+              jv = make_int4(0, 0, 0, 0);
+              xv = make_float4(0.f, 0.f, 0.f, 0.f);
+              if (e0 + 0 < s.len) { jv.x = __ldg(ip + 0); xv.x = dp[0]; }
+              if (e0 + 1 < s.len) { jv.y = __ldg(ip + 1); xv.y = dp[1]; }
+              if (e0 + 2 < s.len) { jv.z = __ldg(ip + 2); xv.z = dp[2]; }
+            }
           }
         }
       };
-      auto compute_step = [&](const Seg& s, int st, const int4& jv, const float4& xv) {
-        const int q = st * 32 + lane;
-        const int e0 = q * 4 - s.head;
-        float* dq = a.data + (s.abeg + 4 * q);
+      auto compute_step = [&](const Seg& s, int st, float* dq, const int4& jv, const float4& xv) {
         if (interior(s, st)) {
-          const float4 r = quad(std::false_type{}, jv, xv, s.scale, e0, s.len);
+          const float4 r = quad(std::false_type{}, jv, xv, s.scale, 0, s.len);
           // x'' is written once and not read again by this pass: streaming stores (evict-first in L2) keep the
           // look-ahead's lines resident (3.257 -> 3.185 ms)
           if (!MOM) st_once(reinterpret_cast<float4*>(dq), r);
-        } else if (q < s.nq) {
-          const float4 r = quad(std::true_type{}, jv, xv, s.scale, e0, s.len);
-          if (MOM) {
-            // nothing is written back
-          } else if (e0 >= 0 && e0 + 4 <= s.len) {
-            *reinterpret_cast<float4*>(dq) = r;             // (plain: the line is shared with a neighbouring segment)
-          } else {
-            if ((unsigned)(e0 + 0) < (unsigned)s.len) dq[0] = r.x;
-            if ((unsigned)(e0 + 1) < (unsigned)s.len) dq[1] = r.y;
-            if ((unsigned)(e0 + 2) < (unsigned)s.len) dq[2] = r.z;
-            if ((unsigned)(e0 + 3) < (unsigned)s.len) dq[3] = r.w;
+        } else {
+          const int q = st * 32 + lane;
+          const int e0 = q * 4 - s.head;
+          if (q < s.nq) {
+            const float4 r = quad(std::true_type{}, jv, xv, s.scale, e0, s.len);
+            if (MOM) {
+              // nothing is written back
+            } else if (e0 >= 0 && e0 + 4 <= s.len) {
+              *reinterpret_cast<float4*>(dq) = r;           // (plain: the line is shared with a neighbouring segment)
+            } else {
+              if ((unsigned)(e0 + 0) < (unsigned)s.len) dq[0] = r.x;
+              if ((unsigned)(e0 + 1) < (unsigned)s.len) dq[1] = r.y;
+              if ((unsigned)(e0 + 2) < (unsigned)s.len) dq[2] = r.z;
+              if ((unsigned)(e0 + 3) < (unsigned)s.len) dq[3] = r.w;
+            }
           }
         }
       };
@@ -610,10 +620,17 @@ __device__ __forceinline__ void fused_stream_body(const FusedArgs& a, uint32_t* 
         while (++ri < kFuRowsPerGrab) { S = seg_of(ri); if (S.nq) break; }
         int4 jn = make_int4(0, 0, 0, 0);
         float4 xn4 = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (ri < kFuRowsPerGrab) load_step(S, 0, jn, xn4);
+        // kRun: the lane's quad address is carried from step to step (log-scale set: 3.139 -> 3.083 ms).  The
+        // kernels with the linear-scale set have no register to spare for it (measured: +6 % / +9 % from
+        // spills) and rebuild the address from the step number.
+        constexpr bool kRun = LOG && !LIN;
+        auto quad_ptr = [&](const Seg& s, int st) -> float* { return a.data + (s.abeg + 4 * (st * 32 + lane)); };
+        float* dpc = a.data;
+        if (ri < kFuRowsPerGrab) { dpc = quad_ptr(S, 0); load_step(S, 0, dpc, jn, xn4); }
         while (ri < kFuRowsPerGrab) {
           const int nsteps = (S.nq + 31) >> 5;
           int nri = ri;
+          float* dpn = dpc;
           // the next row's segment (of this grab or the first of the next) goes to L2 now
           if (ri + 1 < kFuRowsPerGrab) l2_prefetch(mbeg, mend, ri + 1);
           else if (next_ok) l2_prefetch(nbeg, nend, 0);
@@ -623,15 +640,17 @@ __device__ __forceinline__ void fused_stream_body(const FusedArgs& a, uint32_t* 
             const float4 xc = xn4;
             if ((st & 3) == 0 && st * 128 + kFuDist < S.head + S.len) lookahead_in(S.abeg, S.head + S.len, st);
             if (st + 1 < nsteps) {
-              load_step(S, st + 1, jn, xn4);
+              load_step(S, st + 1, kRun ? dpc + 128 : quad_ptr(S, st + 1), jn, xn4);
             } else {                                      // prefetch the next segment's first step
               Seg N;
               N.nq = 0;
               while (++nri < kFuRowsPerGrab) { N = seg_of(nri); if (N.nq) break; }
-              if (nri < kFuRowsPerGrab) load_step(N, 0, jn, xn4);
+              if (nri < kFuRowsPerGrab) { dpn = quad_ptr(N, 0); load_step(N, 0, dpn, jn, xn4); }
             }
-            compute_step(S, st, jc, xc);
+            compute_step(S, st, kRun ? dpc : quad_ptr(S, st), jc, xc);
+            if (kRun) dpc += 128;
           }
+          if (kRun) dpc = dpn;
           ri = nri;
           if (ri < kFuRowsPerGrab) S = seg_of(ri);
         }
