@@ -372,6 +372,30 @@ int rsc_hvg_select(int32_t n_genes, const double* gene_mean, const double* gene_
                    int32_t* out_count, void* ws, size_t ws_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------------
+ * rsc_hvg_select_no_alloc — rsc_hvg_select without a workspace argument, for callers that can
+ * neither allocate device memory nor hand one in (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc).  Same operation, same kernels, same arguments and
+ * outputs as rsc_hvg_select; the kernels' scratch lives in a device array
+ * built into the library:
+ *   * at most RSC_HVG_NO_ALLOC_MAX_GENES genes (2 MiB of device memory, held by every GPU
+ *     that loads the library until the process exits); more genes -> RSC_ERR_INVALID_ARG,
+ *     nothing is launched (use rsc_hvg_select with your own workspace);
+ *   * the call allocates and frees nothing (no cudaMalloc / cudaFree, no allocating library
+ *     routine); the first call on a device looks the array's address up once;
+ *   * all calls on one device share the array: calls that OVERLAP on the GPU (different
+ *     streams, concurrent graph replays) race on it and must be serialised by the caller.
+ *     Nothing in it carries over between calls (every element is written before it is read).
+ * rsc_hvg_select_no_alloc_max_genes() returns the limit the library was built with.
+ * ------------------------------------------------------------------------------- */
+#define RSC_HVG_NO_ALLOC_MAX_GENES 65536
+int32_t rsc_hvg_select_no_alloc_max_genes(void);
+int rsc_hvg_select_no_alloc(int32_t n_genes, const double* gene_mean, const double* gene_var,
+                            int32_t n_top, int32_t n_bins, int flags,
+                            double* out_mean_t, double* out_disp, double* out_disp_norm,
+                            int32_t* out_bin, uint8_t* out_mask, int32_t* out_indices,
+                            int32_t* out_count, void* stream);
+
+/* ---------------------------------------------------------------------------------
  * rsc_preprocess — the whole chain in one call on device-resident data:
  * rsc_qc_metrics -> rsc_normalize_log1p_moments -> rsc_hvg_select (fed with the
  * linear-scale moments when hvg_on_linear != 0, else the log-scale ones; DESIGN.md

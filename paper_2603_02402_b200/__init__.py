@@ -14,6 +14,7 @@ from .binding import (  # noqa: F401
     rsc_normalize_total, rsc_preprocess, rsc_qc_metrics, rsc_version,
     rsc_filter_masks, rsc_subset_csr, rsc_scale_dense, rsc_gram_cov, rsc_pca_transform,
     rsc_hvg_select_cell_ranger, rsc_hvg_merge_batches, rsc_hvg_select_batched, rsc_hvg_cutoffs,
+    rsc_hvg_select_no_alloc, rsc_hvg_select_no_alloc_max_genes,
 )
 
 __all__ = [
@@ -21,4 +22,5 @@ __all__ = [
     "rsc_log1p", "rsc_moments_finalize", "rsc_normalize_log1p_moments", "rsc_normalize_total", "rsc_preprocess",
     "rsc_qc_metrics", "rsc_version", "rsc_filter_masks", "rsc_subset_csr", "rsc_scale_dense", "rsc_gram_cov", "rsc_pca_transform",
     "rsc_hvg_select_cell_ranger", "rsc_hvg_merge_batches", "rsc_hvg_select_batched", "rsc_hvg_cutoffs",
+    "rsc_hvg_select_no_alloc", "rsc_hvg_select_no_alloc_max_genes",
 ]

@@ -39,6 +39,7 @@ EXPORTS = [
     "rsc_normalize_log1p_moments_workspace_bytes", "rsc_normalize_log1p_moments",
     "rsc_moments_finalize",
     "rsc_hvg_select_workspace_bytes", "rsc_hvg_select",
+    "rsc_hvg_select_no_alloc_max_genes", "rsc_hvg_select_no_alloc",
     "rsc_filter_masks", "rsc_subset_csr_workspace_bytes", "rsc_subset_csr_plan", "rsc_subset_csr_fill",
     "rsc_scale_dense_workspace_bytes", "rsc_scale_dense", "rsc_hvg_cutoffs",
     "rsc_gram_cov_workspace_bytes", "rsc_gram_cov", "rsc_pca_transform_workspace_bytes", "rsc_pca_transform",
@@ -137,6 +138,9 @@ def lib() -> C.CDLL:
     L.rsc_normalize_log1p_moments.argtypes = [p, flt, p, p, p, C.c_int, C.c_int, p, p, p, p, p, p, sz, p]
     L.rsc_moments_finalize.argtypes = [i32, i64, C.c_int, p, p, p, p, p]
     L.rsc_hvg_select.argtypes = [i32, p, p, i32, i32, C.c_int, p, p, p, p, p, p, p, p, sz, p]
+    L.rsc_hvg_select_no_alloc.argtypes = [i32, p, p, i32, i32, C.c_int, p, p, p, p, p, p, p, p]
+    L.rsc_hvg_select_no_alloc_max_genes.argtypes = []
+    L.rsc_hvg_select_no_alloc_max_genes.restype = i32
     L.rsc_preprocess.argtypes = [p, p, p, p, p, sz, p]
     L.rsc_preprocess_host.argtypes = [p, p, p, p, p, p, sz, p]
     _lib = L
@@ -357,6 +361,35 @@ def rsc_hvg_select(gene_mean: torch.Tensor, gene_var: torch.Tensor, n_top: int, 
                             _ptr(out["mean_t"]), _ptr(out["disp"]), _ptr(out["disp_norm"]),
                             _ptr(out["bin"]), _ptr(out["mask"]), _ptr(out["indices"]),
                             _ptr(out["count"]), _ptr(ws), ws.numel(), _stream(stream)))
+    return out
+
+
+def rsc_hvg_select_no_alloc_max_genes() -> int:
+    return int(lib().rsc_hvg_select_no_alloc_max_genes())
+
+
+def rsc_hvg_select_no_alloc(gene_mean: torch.Tensor, gene_var: torch.Tensor, n_top: int, n_bins: int = 20,
+                            flags: int = RSC_HVG_SEURAT_LOG, out: Optional[dict] = None, stream=None) -> dict:
+    """rsc_hvg_select on the library's built-in scratch array: the C call allocates nothing.  `out`
+    (tensors keyed as rsc_hvg_select returns them) lets the caller pre-allocate the outputs too."""
+    if not gene_mean.is_cuda:
+        raise RscError(RSC_ERR_INVALID_ARG, "device tensors required (no CPU fallback)")
+    assert gene_mean.dtype == torch.float64 and gene_var.dtype == torch.float64
+    L, dev, G = lib(), gene_mean.device, gene_mean.shape[0]
+    if out is None:
+        out = dict(
+            mean_t=torch.empty(G, dtype=torch.float64, device=dev),
+            disp=torch.empty(G, dtype=torch.float64, device=dev),
+            disp_norm=torch.empty(G, dtype=torch.float64, device=dev),
+            bin=torch.empty(G, dtype=torch.int32, device=dev),
+            mask=torch.empty(G, dtype=torch.uint8, device=dev),
+            indices=torch.full((G,), -1, dtype=torch.int32, device=dev),
+            count=torch.zeros(1, dtype=torch.int32, device=dev),
+        )
+    _check(L.rsc_hvg_select_no_alloc(G, _ptr(gene_mean), _ptr(gene_var), n_top, n_bins, flags,
+                                     _ptr(out.get("mean_t")), _ptr(out.get("disp")), _ptr(out.get("disp_norm")),
+                                     _ptr(out.get("bin")), _ptr(out["mask"]), _ptr(out.get("indices")),
+                                     _ptr(out["count"]), _stream(stream)))
     return out
 
 
