@@ -662,6 +662,12 @@ single_pass_kernel(const SingleArgs a) {
 // slower), the sampled columns give the entries per block of kSpBlock genes.
 __global__ void __launch_bounds__(256)
 single_sample_kernel(SingleArgs a, int n_samples) {
+  // the column histogram is collected per CTA in shared memory first: 3 M adds onto ~120 global addresses
+  // took 0.8 ms
+  __shared__ unsigned int hist[kSpMaxGenes / kSpBlock + 1];
+  const int n_hist = a.n_cols / kSpBlock + 1;
+  for (int i = threadIdx.x; i < n_hist; i += blockDim.x) hist[i] = 0u;
+  __syncthreads();
   const int lane = threadIdx.x & 31;
   const int wid = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5);
   const int n_warps = (int)((gridDim.x * blockDim.x) >> 5);
@@ -671,7 +677,7 @@ single_sample_kernel(SingleArgs a, int n_samples) {
     long long t = 0;
     for (int64_t p = beg + lane; p < end; p += 32) {
       t += (long long)a.data[p];
-      atomicAdd(&a.col_hist[min(max(a.indices[p], 0), a.n_cols - 1) / kSpBlock], 1u);
+      atomicAdd(&hist[min(max(a.indices[p], 0), a.n_cols - 1) / kSpBlock], 1u);
     }
     t = warp_sum(t);
     if (lane == 0 && t > 0) {
@@ -680,6 +686,9 @@ single_sample_kernel(SingleArgs a, int n_samples) {
       atomicAdd(&a.plan->depth_hist[min(max(e - 1 + 32, 0), 63)], 1u);
     }
   }
+  __syncthreads();
+  for (int i = threadIdx.x; i < n_hist; i += blockDim.x)
+    if (hist[i]) atomicAdd(&a.col_hist[i], hist[i]);
 }
 
 __global__ void single_plan_kernel(SingleArgs a, int n_samples) {

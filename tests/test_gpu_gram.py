@@ -72,7 +72,10 @@ def test_gram_cov_hvg_subset_of_cfg1():
 
 
 @pytest.mark.parametrize("n,G,k,seed,center", [(300, 100, 5, 0, True), (1000, 300, 50, 1, True), (777, 129, 33, 2, False),
-                                               (2000, 500, 128, 3, True), (64, 40, 1, 4, True)])
+                                               (2000, 500, 128, 3, True), (64, 40, 1, 4, True),
+                                               # large loading tables (0.8 - 3 MB: served from L2), a short matrix
+                                               (1500, 4000, 50, 5, True), (500, 2300, 128, 6, True),
+                                               (200, 6000, 128, 7, False), (33, 4000, 50, 8, False)])
 def test_pca_transform(n, G, k, seed, center):
     """rsc_pca_transform against oracle_np.pca_transform (PAPER.md:L95 Z = XV - 1 mu^T V).  Bound: V
     travels as float32 (6e-8 per term) and the result is rounded to float32."""
