@@ -169,7 +169,7 @@ fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid, f
     {
       // log-scale set: a window of kLogBinades binades [2^L, 2^(L + kLogBinades)).  The bottom
       // is the binade of the smallest x'' of the data -- a unit count in the deepest cell --
-      // taken robustly: the n / 4096 deepest cells are ignored (their small values take the
+      // taken robustly: the ~n / 65 536 deepest cells are ignored (their small values take the
       // global path), so one outlier cell cannot drag the window away from the bulk.  Never
       // above the top 2^E > log1p(target_sum) (the largest x'' non-negative data can produce),
       // and never below 2^-2: log1p_ge_quarter of an x' < 0.25 is < 0.2232, so such a value
@@ -178,7 +178,10 @@ fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid, f
       frexp(log1p(ts) * 1.000001, &E);
       int L = E - kLogBinades;
       {
-        const unsigned long long skip = (unsigned long long)n_rows / 4096ull;
+        // (n / 65 536 cells, at least 8 when the matrix has 4 096 cells or more; was n / 4 096: fewer values on
+        // the order-dependent global path, and with 24 deep rows of ~100 us each config 2 had a 25 % tail)
+        unsigned long long skip = (unsigned long long)n_rows / 65536ull;
+        if (skip < 8ull) skip = (unsigned long long)n_rows / 512ull < 8ull ? (unsigned long long)n_rows / 512ull : 8ull;
         unsigned long long below = 0ull;
         for (int b = 0; b < 64; ++b) {
           below += plan->depth_hist[b];
