@@ -178,8 +178,9 @@ fused_plan_kernel(FusedPlan* plan, int G, int K, int fine_per_group, int grid, f
       frexp(log1p(ts) * 1.000001, &E);
       int L = E - kLogBinades;
       {
-        // (n / 65 536 cells, at least 8 when the matrix has 4 096 cells or more; was n / 4 096: fewer values on
-        // the order-dependent global path, and with 24 deep rows of ~100 us each config 2 had a 25 % tail)
+        // (n / 65 536 cells, at least 8 when the matrix has 4 096 cells or more; was n / 4 096.  Every unit count of
+        // an ignored cell takes the per-entry slow path, ~100 us per row segment for one warp: with 24 such rows
+        // config 2 had a straggler tail of 25 %; fewer values on the order-dependent global path, too)
         unsigned long long skip = (unsigned long long)n_rows / 65536ull;
         if (skip < 8ull) skip = (unsigned long long)n_rows / 512ull < 8ull ? (unsigned long long)n_rows / 512ull : 8ull;
         unsigned long long below = 0ull;

@@ -348,29 +348,6 @@ __device__ __noinline__ float4 quad_rare(const AccCtx& c, int4 jv, float4 xv, fl
       acc_quad_wide(c.sb_lin, so, an);
     }
   } else {
-    if (LOG && !LIN) {
-      // Log-scale set only, every value computed above is the right one (x' >= 0.25): the entries outside
-      // the window go to the global double sums from here, in line -- what acc3_slow does, without the call
-      // chain per entry.  A deep cell (all of its unit counts below the window) otherwise keeps one warp busy
-      // for ~100 us; such a row near the end of the pass was a straggler tail of that length (config 2: 25 %).
-      bool direct = true;
-#pragma unroll
-      for (int k = 0; k < 4; ++k) direct = direct && (MOM || xn[k] >= 0.25f || !((valid_mask >> k) & 1u));
-      if (direct) {
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          if (!((valid_mask >> k) & 1u) || xl[k] == 0.0f) continue;
-          if (in_window_log(tl[k])) {
-            acc3_word(c.sb_log + slot[k] * (kLogWords * 4u), __float2uint_rz(tl[k]));
-          } else {
-            const double d = (double)xl[k];
-            atomicAdd(c.S1log + c.g0 + slot[k], d);
-            atomicAdd(c.S2log + c.g0 + slot[k], d * d);
-          }
-        }
-        return make_float4(xl[0], xl[1], xl[2], xl[3]);
-      }
-    }
 #pragma unroll
     for (int k = 0; k < 4; ++k)
       if ((valid_mask >> k) & 1u) xl[k] = entry_any<LOG, LIN, MOM>(c, j[k], x[k], scale);
